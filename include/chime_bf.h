@@ -1,0 +1,123 @@
+/*
+ * chime_bf.h -- C-ABI boundary of the B200-native CHIME/FRB hybrid beamformer hot path.
+ *
+ * What the library computes (arXiv:1702.04728; line numbers are /root/reference/PAPER.md):
+ *   input   4+4-bit complex baseband, 2048 inputs (2 pol x 4 cylinders x 256 N-S feeds) per
+ *           390 kHz coarse channel at 2.56 us cadence            (Table 1; sec. 2, :47)
+ *   a1-a2   unpack, per-input complex gain                        (:40-41, :47; gains: BASELINE.json)
+ *   a3-a4   zero-padded N-S spatial DFT (256 -> NP bins) and selection of the 256 bins nearest
+ *           the desired pointings                                 (sec. 3.1, :59-61; eq. (1),(2), :67-78)
+ *   a5      exact phasing of the 4 cylinders into 4 E-W beams     (:18, :51, :80)
+ *   a6      corner turn time-slowest -> time-fastest              (the paper's 2nd kernel, :51)
+ *   a7      U-point DFT over every U consecutive time samples     (sec. 3.2, :51, :84-86)
+ *   a8-a10  |.|^2, sum 2 polarisations, sum U/16 adjacent fine channels, sum 3 blocks,
+ *           rescale to 8-bit integers                             (:37-42, :53)
+ *   output  1024 beams (4 E-W x 256 N-S) x 16 fine channels per coarse channel every
+ *           3*U samples (0.983 ms for U = 128), uint8.
+ * The conventions the paper leaves open (nibble order, sign of the DFTs, grouping of fine channels,
+ * normalisation, rounding of the index table) are the readings A1-A16 listed in DESIGN.md.
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.  All entry points
+ * are thread-compatible (one thread per plan at a time).  Pointers are marked HOST or DEVICE.
+ */
+#ifndef CHIME_BF_H
+#define CHIME_BF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CHIME_BF_N_FEED 256   /* N-S feeds per cylinder */
+#define CHIME_BF_N_CYL 4      /* cylinders */
+#define CHIME_BF_N_POL 2      /* polarisations */
+#define CHIME_BF_N_INPUT 2048 /* input index i = (pol*4 + cyl)*256 + feed */
+#define CHIME_BF_N_EW 4       /* E-W formed beams */
+#define CHIME_BF_N_BEAM 1024  /* beam index b = ew*256 + ns */
+#define CHIME_BF_N_FINE 16    /* fine channels per coarse channel in the output */
+#define CHIME_BF_N_INT 3      /* U-sample blocks integrated per output frame */
+
+/* return codes of the int-returning calls */
+#define CHIME_BF_OK 0
+#define CHIME_BF_E_INVALID_ARG (-1)
+#define CHIME_BF_E_ALIGNMENT (-2)
+#define CHIME_BF_E_CUDA (-3)
+#define CHIME_BF_E_UNSUPPORTED (-4)
+
+typedef struct chime_bf_plan chime_bf_plan; /* opaque; owns its device tables */
+
+/*
+ * Plan creation, north-star form.  Channel k has centre frequency 800 - k*0.390625 MHz;
+ * n_time = 49152 samples per execute; f_ref = 600 MHz; scale 1/64, offset 128; feed spacing
+ * 0.3048 m; cylinder spacing 22 m.
+ *   n_coarse    number of coarse channels C (>= 1)
+ *   gains       HOST, [C][2048][2] float (re, im), copied; NULL = unit gains.  Zero = flagged input.
+ *   ew_angles   HOST, [4] double, E-W beam angles in degrees, copied
+ *   zero_pad    NP, padded N-S transform length: 256, 512 or 1024
+ *   upchan_len  U, up-channelisation length: 128 or 256 (fine channels out = 16, D = U/16)
+ * Returns NULL on error; chime_bf_last_error() tells why.  Binds to the current CUDA device.
+ */
+chime_bf_plan *chime_bf_plan_create(int n_coarse, const float *gains, const double *ew_angles,
+                                    int zero_pad, int upchan_len);
+
+/* Extended form: everything the five BASELINE.json configurations vary. */
+typedef struct {
+    int n_coarse;                /* C */
+    const double *freq_mhz;      /* HOST [C] centre frequencies in MHz; NULL = 800 - k*0.390625 */
+    const float *gains;          /* HOST [C][2048][2] or NULL */
+    const double *ew_angles_deg; /* HOST [4] */
+    int zero_pad;                /* NP in {256, 512, 1024} */
+    int upchan_len;              /* U in {128, 256} */
+    int n_time;                  /* samples per execute; multiple of 3*U */
+    double f_ref_mhz;            /* reference frequency of the desired pointings (A2); <= 0 -> 600 */
+    const double *ns_sin_theta;  /* HOST [256] explicit desired pointings sin(theta_m), or NULL */
+    float scale, offset;         /* u8 = sat(rne(I*scale + offset)); scale <= 0 -> 1/64, 128 */
+    double feed_spacing_m;       /* <= 0 -> 0.3048 */
+    double cyl_spacing_m;        /* <= 0 -> 22 */
+} chime_bf_params;
+
+chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *params);
+
+/*
+ * One pass of the whole hot path (a1-a10) over [C][n_time] samples, asynchronous on `cuda_stream`
+ * (a cudaStream_t / CUstream passed as void*; NULL = legacy default stream).  Never synchronises,
+ * never allocates.
+ *   in_u8    DEVICE, [C][n_time][2048] bytes, byte = ((re+8) << 4) | (im+8); 16-byte aligned;
+ *            caller-owned, read-only
+ *   out_u8   DEVICE, [C][n_time/(3U)][4][256][16] bytes; 16-byte aligned; caller-owned
+ * Returns CHIME_BF_OK or a negative code.
+ */
+int chime_bf_execute(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8, uint8_t *out_u8);
+
+/* Same pass, but writes the pre-quantisation float intensities I (a9) in the same layout. */
+int chime_bf_execute_f32(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8,
+                         float *out_f32);
+
+/* Convenience: HOST buffers in and out; the library stages them through device memory
+ * (allocated on first use, owned by the plan), runs execute on `cuda_stream` and synchronises it. */
+int chime_bf_execute_host(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8_host,
+                          uint8_t *out_u8_host);
+
+/* Copy of the clamped N-S bin index table J (eq. (1),(2)): HOST out, [C][256] int32. */
+int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out);
+
+/* Step a1 alone: DEVICE in_u8 [n_bytes] -> DEVICE out_re_im [n_bytes][2] int8 (re, im). */
+int chime_bf_debug_unpack(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8,
+                          size_t n_bytes, int8_t *out_re_im);
+
+/* Shape queries (so bindings need not re-derive them). */
+int chime_bf_n_frames(const chime_bf_plan *plan);       /* n_time / (3U) */
+size_t chime_bf_in_bytes(const chime_bf_plan *plan);    /* C * n_time * 2048 */
+size_t chime_bf_out_elems(const chime_bf_plan *plan);   /* C * n_frames * 1024 * 16 */
+int chime_bf_launches_per_execute(const chime_bf_plan *plan); /* kernels launched by one execute */
+
+void chime_bf_destroy(chime_bf_plan *plan); /* NULL-safe */
+
+const char *chime_bf_last_error(void); /* thread-local, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHIME_BF_H */

@@ -1,0 +1,229 @@
+"""paper_1702_04728_b200 -- thin Python binding of libchime_bf.so (include/chime_bf.h).
+
+Argument marshalling only: every step of the beamformer runs in the CUDA kernels of csrc/.
+PyTorch is used for device memory and streams.  There is no CPU fallback: if the library or a
+CUDA device is missing, calls raise.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from .build import LIB_PATH, build_library
+
+N_FEED, N_CYL, N_POL, N_INPUT, N_EW, N_BEAM, N_FINE, N_INT = 256, 4, 2, 2048, 4, 1024, 16, 3
+EW_ANGLES_DEG = (-0.6, -0.2, 0.2, 0.6)
+
+EXPORTS = [
+    "chime_bf_plan_create", "chime_bf_plan_create_ex", "chime_bf_execute", "chime_bf_execute_f32",
+    "chime_bf_execute_host", "chime_bf_get_ns_index", "chime_bf_debug_unpack", "chime_bf_n_frames",
+    "chime_bf_in_bytes", "chime_bf_out_elems", "chime_bf_launches_per_execute", "chime_bf_destroy",
+    "chime_bf_last_error",
+]
+
+
+class chime_bf_params(ctypes.Structure):
+    _fields_ = [
+        ("n_coarse", ctypes.c_int),
+        ("freq_mhz", ctypes.POINTER(ctypes.c_double)),
+        ("gains", ctypes.POINTER(ctypes.c_float)),
+        ("ew_angles_deg", ctypes.POINTER(ctypes.c_double)),
+        ("zero_pad", ctypes.c_int),
+        ("upchan_len", ctypes.c_int),
+        ("n_time", ctypes.c_int),
+        ("f_ref_mhz", ctypes.c_double),
+        ("ns_sin_theta", ctypes.POINTER(ctypes.c_double)),
+        ("scale", ctypes.c_float),
+        ("offset", ctypes.c_float),
+        ("feed_spacing_m", ctypes.c_double),
+        ("cyl_spacing_m", ctypes.c_double),
+    ]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree C-ABI library (must have been built: __graft_entry__.build())."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                           "(there is no fallback path)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    lib.chime_bf_plan_create.restype = vp
+    lib.chime_bf_plan_create.argtypes = [ci, vp, vp, ci, ci]
+    lib.chime_bf_plan_create_ex.restype = vp
+    lib.chime_bf_plan_create_ex.argtypes = [ctypes.POINTER(chime_bf_params)]
+    lib.chime_bf_execute.restype = ci
+    lib.chime_bf_execute.argtypes = [vp, vp, vp, vp]
+    lib.chime_bf_execute_f32.restype = ci
+    lib.chime_bf_execute_f32.argtypes = [vp, vp, vp, vp]
+    lib.chime_bf_execute_host.restype = ci
+    lib.chime_bf_execute_host.argtypes = [vp, vp, vp, vp]
+    lib.chime_bf_get_ns_index.restype = ci
+    lib.chime_bf_get_ns_index.argtypes = [vp, vp]
+    lib.chime_bf_debug_unpack.restype = ci
+    lib.chime_bf_debug_unpack.argtypes = [vp, vp, vp, ctypes.c_size_t, vp]
+    lib.chime_bf_n_frames.restype = ci
+    lib.chime_bf_n_frames.argtypes = [vp]
+    lib.chime_bf_in_bytes.restype = ctypes.c_size_t
+    lib.chime_bf_in_bytes.argtypes = [vp]
+    lib.chime_bf_out_elems.restype = ctypes.c_size_t
+    lib.chime_bf_out_elems.argtypes = [vp]
+    lib.chime_bf_launches_per_execute.restype = ci
+    lib.chime_bf_launches_per_execute.argtypes = [vp]
+    lib.chime_bf_destroy.restype = None
+    lib.chime_bf_destroy.argtypes = [vp]
+    lib.chime_bf_last_error.restype = ctypes.c_char_p
+    lib.chime_bf_last_error.argtypes = []
+    _lib = lib
+    return lib
+
+
+def last_error():
+    return load_library().chime_bf_last_error().decode()
+
+
+class ChimeBfError(RuntimeError):
+    pass
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+class Plan:
+    """Owns a chime_bf_plan*.  Methods carry the C-ABI names (chime_bf_ prefix dropped)."""
+
+    def __init__(self, handle, n_coarse, zero_pad, upchan_len, n_time):
+        self._h = handle
+        self.n_coarse, self.zero_pad, self.upchan_len, self.n_time = n_coarse, zero_pad, upchan_len, n_time
+        lib = load_library()
+        self.n_frames = lib.chime_bf_n_frames(handle)
+        self.in_bytes = lib.chime_bf_in_bytes(handle)
+        self.out_elems = lib.chime_bf_out_elems(handle)
+        self.launches_per_execute = lib.chime_bf_launches_per_execute(handle)
+        self.in_shape = (n_coarse, n_time, N_INPUT)
+        self.out_shape = (n_coarse, self.n_frames, N_EW, N_FEED, N_FINE)
+
+    def _check(self, rc):
+        if rc != 0:
+            raise ChimeBfError(f"chime_bf error {rc}: {last_error()}")
+
+    def _check_in(self, in_u8):
+        import torch
+        if not (in_u8.is_cuda and in_u8.dtype == torch.uint8 and in_u8.is_contiguous()
+                and in_u8.numel() == self.in_bytes):
+            raise ValueError(f"in_u8 must be a contiguous CUDA uint8 tensor of {self.in_bytes} bytes")
+
+    def execute(self, in_u8, out_u8=None, stream=None):
+        import torch
+        self._check_in(in_u8)
+        if out_u8 is None:
+            out_u8 = torch.empty(self.out_shape, dtype=torch.uint8, device=in_u8.device)
+        assert out_u8.is_cuda and out_u8.dtype == torch.uint8 and out_u8.numel() == self.out_elems
+        self._check(load_library().chime_bf_execute(self._h, _stream_ptr(stream), in_u8.data_ptr(),
+                                                    out_u8.data_ptr()))
+        return out_u8
+
+    def execute_f32(self, in_u8, out_f32=None, stream=None):
+        import torch
+        self._check_in(in_u8)
+        if out_f32 is None:
+            out_f32 = torch.empty(self.out_shape, dtype=torch.float32, device=in_u8.device)
+        assert out_f32.is_cuda and out_f32.dtype == torch.float32 and out_f32.numel() == self.out_elems
+        self._check(load_library().chime_bf_execute_f32(self._h, _stream_ptr(stream), in_u8.data_ptr(),
+                                                        out_f32.data_ptr()))
+        return out_f32
+
+    def execute_host(self, in_u8_host, out_u8_host=None, stream=None):
+        """HOST tensors (ideally pinned) in and out; H2D, kernels and D2H all inside the call."""
+        import torch
+        assert (not in_u8_host.is_cuda) and in_u8_host.dtype == torch.uint8 and in_u8_host.is_contiguous()
+        assert in_u8_host.numel() == self.in_bytes
+        if out_u8_host is None:
+            out_u8_host = torch.empty(self.out_shape, dtype=torch.uint8).pin_memory()
+        assert out_u8_host.numel() == self.out_elems and out_u8_host.is_contiguous()
+        self._check(load_library().chime_bf_execute_host(self._h, _stream_ptr(stream),
+                                                         in_u8_host.data_ptr(), out_u8_host.data_ptr()))
+        return out_u8_host
+
+    def get_ns_index(self):
+        J = np.zeros((self.n_coarse, N_FEED), dtype=np.int32)
+        self._check(load_library().chime_bf_get_ns_index(self._h, J.ctypes.data))
+        return J
+
+    def debug_unpack(self, in_u8, stream=None):
+        import torch
+        assert in_u8.is_cuda and in_u8.dtype == torch.uint8 and in_u8.is_contiguous()
+        out = torch.empty((in_u8.numel(), 2), dtype=torch.int8, device=in_u8.device)
+        self._check(load_library().chime_bf_debug_unpack(self._h, _stream_ptr(stream), in_u8.data_ptr(),
+                                                         in_u8.numel(), out.data_ptr()))
+        return out
+
+    def destroy(self):
+        if self._h:
+            load_library().chime_bf_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def plan_create(n_coarse, gains=None, ew_angles=EW_ANGLES_DEG, zero_pad=512, upchan_len=128):
+    """chime_bf_plan_create: north-star form (f_k = 800 - k*0.390625 MHz, n_time = 49152)."""
+    lib = load_library()
+    g = None if gains is None else np.ascontiguousarray(gains, dtype=np.float32)
+    if g is not None and g.size != n_coarse * N_INPUT * 2:
+        raise ValueError("gains must have shape [n_coarse][2048][2]")
+    ew = np.ascontiguousarray(ew_angles, dtype=np.float64)
+    if ew.size != N_EW:
+        raise ValueError("ew_angles must have 4 entries")
+    h = lib.chime_bf_plan_create(n_coarse, None if g is None else g.ctypes.data, ew.ctypes.data,
+                                 zero_pad, upchan_len)
+    if not h:
+        raise ChimeBfError(last_error())
+    return Plan(h, n_coarse, zero_pad, upchan_len, 49152)
+
+
+def plan_create_ex(n_coarse, freq_mhz=None, gains=None, ew_angles=EW_ANGLES_DEG, zero_pad=512,
+                   upchan_len=128, n_time=49152, f_ref_mhz=0.0, ns_sin_theta=None, scale=0.0, offset=0.0,
+                   feed_spacing_m=0.0, cyl_spacing_m=0.0):
+    """chime_bf_plan_create_ex: every knob of chime_bf_params (zeros select the defaults)."""
+    lib = load_library()
+    keep = []
+
+    def dptr(a, n, ctype, npt):
+        if a is None:
+            return None
+        a = np.ascontiguousarray(a, dtype=npt)
+        if a.size != n:
+            raise ValueError(f"expected {n} elements, got {a.size}")
+        keep.append(a)
+        return a.ctypes.data_as(ctypes.POINTER(ctype))
+
+    p = chime_bf_params()
+    p.n_coarse = n_coarse
+    p.freq_mhz = dptr(freq_mhz, n_coarse, ctypes.c_double, np.float64)
+    p.gains = dptr(gains, n_coarse * N_INPUT * 2, ctypes.c_float, np.float32)
+    p.ew_angles_deg = dptr(ew_angles, N_EW, ctypes.c_double, np.float64)
+    p.zero_pad, p.upchan_len, p.n_time = zero_pad, upchan_len, n_time
+    p.f_ref_mhz = f_ref_mhz
+    p.ns_sin_theta = dptr(ns_sin_theta, N_FEED, ctypes.c_double, np.float64)
+    p.scale, p.offset = scale, offset
+    p.feed_spacing_m, p.cyl_spacing_m = feed_spacing_m, cyl_spacing_m
+    h = lib.chime_bf_plan_create_ex(ctypes.byref(p))
+    if not h:
+        raise ChimeBfError(last_error())
+    return Plan(h, n_coarse, zero_pad, upchan_len, n_time)

@@ -1,0 +1,344 @@
+// C-ABI of the CHIME/FRB beamformer library (include/chime_bf.h): plan = host-built tables in double
+// precision uploaded once; execute = one fused kernel launch on the caller's stream.
+#include "../../include/chime_bf.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "beamform_kernel.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+void set_err(const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+constexpr double kC0 = 299792458.0;
+constexpr double kPi = 3.14159265358979323846264338327950288;
+
+}  // namespace
+
+struct chime_bf_plan {
+    int C = 0, NP = 0, U = 0, T = 0, R = 0;
+    int device = 0;
+    float scale = 0.f, offset = 0.f, norm = 0.f;
+    std::vector<int32_t> J;  // [C][256]
+    float2 *d_wp = nullptr;
+    int16_t *d_slot = nullptr;
+    int16_t *d_slot_of_m = nullptr;
+    float2 *d_tw_np = nullptr;
+    float2 *d_tw_u = nullptr;
+    // staging for execute_host
+    uint8_t *d_stage_in = nullptr;
+    uint8_t *d_stage_out = nullptr;
+};
+
+namespace {
+
+#define CUDA_TRY(expr)                                                                     \
+    do {                                                                                   \
+        cudaError_t _e = (expr);                                                           \
+        if (_e != cudaSuccess) {                                                           \
+            set_err("%s failed: %s", #expr, cudaGetErrorString(_e));                       \
+            return false;                                                                  \
+        }                                                                                  \
+    } while (0)
+
+// Clamped N-S bin index (eq. (1)+(2); reading A3): round-half-up of
+// x = P (m - 128) f / f_ref, evaluated as one exact integer-by-f product and one division.
+int32_t ns_bin(int P, int m, double f_mhz, double fref_mhz, int NP) {
+    const double x = ((double)(P * (m - 128)) * f_mhz) / fref_mhz;
+    const double fl = std::floor(x);
+    long j = (long)fl + (((x - fl) >= 0.5) ? 1 : 0);
+    j %= NP;
+    if (j < 0) j += NP;
+    return (int32_t)j;
+}
+
+int32_t ns_bin_sintheta(int NP, double f_mhz, double d_m, double s) {
+    const double x = (double)NP * (f_mhz * 1e6) * (d_m / kC0) * s;
+    const double fl = std::floor(x);
+    long j = (long)fl + (((x - fl) >= 0.5) ? 1 : 0);
+    j %= NP;
+    if (j < 0) j += NP;
+    return (int32_t)j;
+}
+
+template <typename T>
+bool upload(T **dst, const std::vector<T> &src) {
+    CUDA_TRY(cudaMalloc((void **)dst, src.size() * sizeof(T)));
+    CUDA_TRY(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return true;
+}
+
+bool build_tables(chime_bf_plan *pl, const chime_bf_params &p, double fref, double d_feed, double d_cyl) {
+    const int C = pl->C, NP = pl->NP, U = pl->U, P = NP / 256;
+    std::vector<float2> wp((size_t)C * 2 * 4 * 4 * 256);
+    std::vector<int16_t> slot((size_t)C * NP), slot_of_m((size_t)C * 256);
+    pl->J.resize((size_t)C * 256);
+    for (int c = 0; c < C; ++c) {
+        const double f = p.freq_mhz ? p.freq_mhz[c] : 800.0 - (double)c * 0.390625;
+        // a4: index table, then compaction of the distinct selected bins into slots
+        int32_t *J = &pl->J[(size_t)c * 256];
+        for (int m = 0; m < 256; ++m)
+            J[m] = p.ns_sin_theta ? ns_bin_sintheta(NP, f, d_feed, p.ns_sin_theta[m])
+                                  : ns_bin(P, m, f, fref, NP);
+        int16_t *sl = &slot[(size_t)c * NP];
+        std::fill(sl, sl + NP, (int16_t)-1);
+        for (int m = 0; m < 256; ++m) sl[J[m]] = 0;
+        int16_t ns = 0;
+        for (int j = 0; j < NP; ++j)
+            if (sl[j] == 0) sl[j] = ns++;
+        for (int m = 0; m < 256; ++m) slot_of_m[(size_t)c * 256 + m] = sl[J[m]];
+        // a2+a5 folded: W'[pol][e][cyl][feed] = exp(-2 pi i f x_cyl sin(phi_e)/c0) * g[pol][cyl][feed]
+        for (int e = 0; e < 4; ++e) {
+            const double s = std::sin(p.ew_angles_deg[e] * kPi / 180.0);
+            for (int cy = 0; cy < 4; ++cy) {
+                const double ph = -2.0 * kPi * (f * 1e6) * ((double)cy * d_cyl) * s / kC0;
+                const double wr = std::cos(ph), wi = std::sin(ph);
+                for (int pol = 0; pol < 2; ++pol)
+                    for (int n = 0; n < 256; ++n) {
+                        double gr = 1.0, gi = 0.0;
+                        if (p.gains) {
+                            const float *g = p.gains + (((size_t)c * 2048) + (pol * 4 + cy) * 256 + n) * 2;
+                            gr = g[0];
+                            gi = g[1];
+                        }
+                        wp[((((size_t)c * 2 + pol) * 4 + e) * 4 + cy) * 256 + n] =
+                            make_float2((float)(wr * gr - wi * gi), (float)(wr * gi + wi * gr));
+                    }
+            }
+        }
+    }
+    std::vector<float2> tw_np(NP), tw_u(U);
+    for (int k = 0; k < NP; ++k) {
+        const double a = -2.0 * kPi * (double)k / (double)NP;
+        tw_np[k] = make_float2((float)std::cos(a), (float)std::sin(a));
+    }
+    for (int k = 0; k < U; ++k) {
+        const double a = -2.0 * kPi * (double)k / (double)U;
+        tw_u[k] = make_float2((float)std::cos(a), (float)std::sin(a));
+    }
+    return upload(&pl->d_wp, wp) && upload(&pl->d_slot, slot) && upload(&pl->d_slot_of_m, slot_of_m) &&
+           upload(&pl->d_tw_np, tw_np) && upload(&pl->d_tw_u, tw_u);
+}
+
+template <int P, int RAD>
+bool prepare_kernel() {
+    CUDA_TRY(cudaFuncSetAttribute(chime::beamform_fused_kernel<P, RAD>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)chime::smem_bytes<P>()));
+    return true;
+}
+
+template <int P, int RAD>
+cudaError_t launch(const chime::KernelParams &kp, int n_cta, cudaStream_t st) {
+    chime::beamform_fused_kernel<P, RAD><<<n_cta, chime::kThreads, chime::smem_bytes<P>(), st>>>(kp);
+    return cudaGetLastError();
+}
+
+int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, float *out_f32) {
+    if (!pl || !in || (!out_u8 && !out_f32)) {
+        set_err("execute: null argument");
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    if (((uintptr_t)in & 15) || ((uintptr_t)out_u8 & 15) || ((uintptr_t)out_f32 & 15)) {
+        set_err("execute: buffers must be 16-byte aligned");
+        return CHIME_BF_E_ALIGNMENT;
+    }
+    chime::KernelParams kp;
+    kp.in = reinterpret_cast<const uint32_t *>(in);
+    kp.out_u8 = out_u8;
+    kp.out_f32 = out_f32;
+    kp.wp = pl->d_wp;
+    kp.slot = pl->d_slot;
+    kp.slot_of_m = pl->d_slot_of_m;
+    kp.tw_np = pl->d_tw_np;
+    kp.tw_u = pl->d_tw_u;
+    kp.n_time = pl->T;
+    kp.n_frames = pl->R;
+    kp.norm = pl->norm;
+    kp.qscale = pl->norm * pl->scale;
+    kp.qoffset = pl->offset;
+    const int n_cta = pl->C * pl->R * 4;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaErrorInvalidValue;
+    const int P = pl->NP / 256, RAD = pl->U / 32;
+    if (P == 1 && RAD == 4) e = launch<1, 4>(kp, n_cta, st);
+    else if (P == 2 && RAD == 4) e = launch<2, 4>(kp, n_cta, st);
+    else if (P == 4 && RAD == 4) e = launch<4, 4>(kp, n_cta, st);
+    else if (P == 1 && RAD == 8) e = launch<1, 8>(kp, n_cta, st);
+    else if (P == 2 && RAD == 8) e = launch<2, 8>(kp, n_cta, st);
+    else if (P == 4 && RAD == 8) e = launch<4, 8>(kp, n_cta, st);
+    if (e != cudaSuccess) {
+        set_err("kernel launch failed: %s", cudaGetErrorString(e));
+        return CHIME_BF_E_CUDA;
+    }
+    return CHIME_BF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *chime_bf_last_error(void) { return g_err; }
+
+chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
+    if (!pp) {
+        set_err("plan_create: null params");
+        return nullptr;
+    }
+    const chime_bf_params &p = *pp;
+    if (p.n_coarse < 1) { set_err("plan_create: n_coarse must be >= 1"); return nullptr; }
+    if (p.zero_pad != 256 && p.zero_pad != 512 && p.zero_pad != 1024) {
+        set_err("plan_create: zero_pad must be 256, 512 or 1024 (got %d)", p.zero_pad);
+        return nullptr;
+    }
+    if (p.upchan_len != 128 && p.upchan_len != 256) {
+        set_err("plan_create: upchan_len must be 128 or 256 (got %d)", p.upchan_len);
+        return nullptr;
+    }
+    if (p.n_time < 3 * p.upchan_len || p.n_time % (3 * p.upchan_len) != 0) {
+        set_err("plan_create: n_time must be a positive multiple of 3*upchan_len (got %d)", p.n_time);
+        return nullptr;
+    }
+    if (!p.ew_angles_deg) { set_err("plan_create: ew_angles is NULL"); return nullptr; }
+    if ((long long)p.n_coarse * (p.n_time / (3 * p.upchan_len)) * 4 > 2147483647LL) {
+        set_err("plan_create: grid too large");
+        return nullptr;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        set_err("plan_create: no CUDA device (this library has no CPU fallback)");
+        return nullptr;
+    }
+    chime_bf_plan *pl = new chime_bf_plan();
+    pl->C = p.n_coarse;
+    pl->NP = p.zero_pad;
+    pl->U = p.upchan_len;
+    pl->T = p.n_time;
+    pl->R = p.n_time / (3 * p.upchan_len);
+    pl->scale = p.scale > 0.f ? p.scale : 1.0f / 64.0f;
+    pl->offset = p.scale > 0.f ? p.offset : 128.0f;
+    pl->norm = (float)(1.0 / (256.0 * 4.0 * (double)p.upchan_len));
+    cudaGetDevice(&pl->device);
+    const double fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
+    const double d_feed = p.feed_spacing_m > 0 ? p.feed_spacing_m : 0.3048;
+    const double d_cyl = p.cyl_spacing_m > 0 ? p.cyl_spacing_m : 22.0;
+    bool ok = build_tables(pl, p, fref, d_feed, d_cyl);
+    ok = ok && prepare_kernel<1, 4>() && prepare_kernel<2, 4>() && prepare_kernel<4, 4>() &&
+         prepare_kernel<1, 8>() && prepare_kernel<2, 8>() && prepare_kernel<4, 8>();
+    if (!ok) {
+        chime_bf_destroy(pl);
+        return nullptr;
+    }
+    return pl;
+}
+
+chime_bf_plan *chime_bf_plan_create(int n_coarse, const float *gains, const double *ew_angles,
+                                    int zero_pad, int upchan_len) {
+    chime_bf_params p;
+    memset(&p, 0, sizeof(p));
+    p.n_coarse = n_coarse;
+    p.gains = gains;
+    p.ew_angles_deg = ew_angles;
+    p.zero_pad = zero_pad;
+    p.upchan_len = upchan_len;
+    p.n_time = 49152;
+    return chime_bf_plan_create_ex(&p);
+}
+
+int chime_bf_execute(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, uint8_t *out_u8) {
+    return run(plan, stream, in_u8, out_u8, nullptr);
+}
+
+int chime_bf_execute_f32(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, float *out_f32) {
+    return run(plan, stream, in_u8, nullptr, out_f32);
+}
+
+int chime_bf_execute_host(chime_bf_plan *pl, void *stream, const uint8_t *in_host, uint8_t *out_host) {
+    if (!pl || !in_host || !out_host) {
+        set_err("execute_host: null argument");
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    const size_t nin = chime_bf_in_bytes(pl), nout = chime_bf_out_elems(pl);
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaSuccess;
+    if (!pl->d_stage_in) e = cudaMalloc((void **)&pl->d_stage_in, nin);
+    if (e == cudaSuccess && !pl->d_stage_out) e = cudaMalloc((void **)&pl->d_stage_out, nout);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_stage_in, in_host, nin, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) {
+        set_err("execute_host: %s", cudaGetErrorString(e));
+        return CHIME_BF_E_CUDA;
+    }
+    const int rc = run(pl, stream, pl->d_stage_in, pl->d_stage_out, nullptr);
+    if (rc != CHIME_BF_OK) return rc;
+    e = cudaMemcpyAsync(out_host, pl->d_stage_out, nout, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        set_err("execute_host: %s", cudaGetErrorString(e));
+        return CHIME_BF_E_CUDA;
+    }
+    return CHIME_BF_OK;
+}
+
+int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out) {
+    if (!plan || !host_out) {
+        set_err("get_ns_index: null argument");
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    memcpy(host_out, plan->J.data(), plan->J.size() * sizeof(int32_t));
+    return CHIME_BF_OK;
+}
+
+int chime_bf_debug_unpack(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, size_t n_bytes,
+                          int8_t *out_re_im) {
+    if (!plan || (n_bytes && (!in_u8 || !out_re_im))) {
+        set_err("debug_unpack: null argument");
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    if (n_bytes == 0) return CHIME_BF_OK;
+    const int threads = 256;
+    const int blocks = (int)std::min<size_t>((n_bytes + threads - 1) / threads, 148 * 16);
+    chime::unpack_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(in_u8, n_bytes, out_re_im);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        set_err("debug_unpack: %s", cudaGetErrorString(e));
+        return CHIME_BF_E_CUDA;
+    }
+    return CHIME_BF_OK;
+}
+
+int chime_bf_n_frames(const chime_bf_plan *plan) { return plan ? plan->R : 0; }
+size_t chime_bf_in_bytes(const chime_bf_plan *plan) {
+    return plan ? (size_t)plan->C * plan->T * 2048 : 0;
+}
+size_t chime_bf_out_elems(const chime_bf_plan *plan) {
+    return plan ? (size_t)plan->C * plan->R * 1024 * 16 : 0;
+}
+int chime_bf_launches_per_execute(const chime_bf_plan *plan) { return plan ? 1 : 0; }
+
+void chime_bf_destroy(chime_bf_plan *pl) {
+    if (!pl) return;
+    cudaFree(pl->d_wp);
+    cudaFree(pl->d_slot);
+    cudaFree(pl->d_slot_of_m);
+    cudaFree(pl->d_tw_np);
+    cudaFree(pl->d_tw_u);
+    cudaFree(pl->d_stage_in);
+    cudaFree(pl->d_stage_out);
+    delete pl;
+}
+
+}  // extern "C"

@@ -1,0 +1,151 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the oracle, element by element, on the same
+seeded bytes.  Tolerances are BASELINE.json's: float intensities within 1e-4 of the beam's mean power;
+uint8 bit-exact except +-1 LSB on at most 0.1 % of entries; index table and unpack bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import synth
+
+pytestmark = pytest.mark.gpu
+
+REL_TOL = 1e-4
+U8_FRAC = 1e-3
+
+
+@pytest.fixture(scope="module")
+def bf():
+    import __graft_entry__ as g
+    g.build()
+    import paper_1702_04728_b200 as bf
+    assert torch.cuda.is_available()
+    return bf
+
+
+def compare_cells(orc, plan, d_in, host_bytes_fn, freqs, gains, cells, np_, U, out_f32=None, out_u8=None):
+    """cells: list of (c, R).  host_bytes_fn(c, R) -> [3U][2048] uint8 numpy."""
+    if out_f32 is None:
+        out_f32 = plan.execute_f32(d_in)
+    if out_u8 is None:
+        out_u8 = plan.execute(d_in)
+    torch.cuda.synchronize()
+    J = plan.get_ns_index()
+    worst, n_diff, n_tot = 0.0, 0, 0
+    for (c, R) in cells:
+        g = None if gains is None else gains[c]
+        I, Jo = orc.cell(host_bytes_fn(c, R), float(freqs[c]), gains=g, np_=np_, U=U)
+        assert np.array_equal(J[c], Jo), f"index table differs for channel {c}"
+        got = out_f32[c, R].cpu().numpy()
+        mean = I.mean(axis=-1, keepdims=True)
+        mean = np.where(mean > 0, mean, 1.0)
+        err = np.abs(got - I) / mean
+        worst = max(worst, float(err.max()))
+        q = orc.quantize(I)
+        d = np.abs(out_u8[c, R].cpu().numpy().astype(int) - q.astype(int))
+        assert d.max() <= 1, f"uint8 differs by {d.max()} LSB in cell {(c, R)}"
+        n_diff += int((d != 0).sum())
+        n_tot += d.size
+    assert worst <= REL_TOL, f"float intensities off by {worst:.3e} of the beam mean power"
+    assert n_diff <= U8_FRAC * n_tot, f"{n_diff}/{n_tot} uint8 entries differ"
+    return worst, n_diff / n_tot
+
+
+def test_cfg0_tiny_full(bf, orc):
+    f = 600.0
+    b = synth.tone_bytes(synth.config_seed(0), f, 768)
+    plan = bf.plan_create_ex(1, freq_mhz=[f], n_time=768)
+    d_in = b.cuda()
+    hb = b.numpy()
+    worst, frac = compare_cells(orc, plan, d_in, lambda c, R: hb[c, 384 * R:384 * (R + 1)], [f], None,
+                                [(0, 0), (0, 1)], 512, 128)
+    out = plan.execute_f32(d_in).cpu().numpy()
+    e, m, g = np.unravel_index(out[0, 0].argmax(), out[0, 0].shape)
+    assert m == 159 and g == 12 and e in (1, 2)
+    print(f"cfg0: worst rel err {worst:.2e}, u8 diff frac {frac:.2e}")
+
+
+def test_unpack_bit_exact(bf, orc):
+    plan = bf.plan_create_ex(1, n_time=384)
+    b = torch.arange(256, dtype=torch.uint8).repeat(37)[:9001].contiguous()   # ragged length
+    got = plan.debug_unpack(b.cuda()).cpu().numpy()
+    assert np.array_equal(got, orc.unpack(b.numpy()))
+    empty = plan.debug_unpack(torch.empty(0, dtype=torch.uint8, device="cuda"))
+    assert empty.numel() == 0
+
+
+def test_index_table_bit_exact_full_band(bf, orc):
+    freqs = synth.chime_freqs_mhz(1024)
+    for NP in (256, 512, 1024):
+        plan = bf.plan_create_ex(1024, zero_pad=NP, n_time=384)
+        J = plan.get_ns_index()
+        for k in range(1024):
+            assert np.array_equal(J[k], orc.ns_index(freqs[k], NP)), (NP, k)
+        plan.destroy()
+
+
+@pytest.mark.parametrize("NP,U", [(256, 128), (512, 128), (1024, 128), (256, 256), (512, 256), (1024, 256)])
+def test_variants_small(bf, orc, NP, U):
+    """cfg4-style sweep at a size the oracle finishes in seconds: 3 channels x 2 frames, random gains
+    with 10 % flagged inputs, 5 % saturated samples."""
+    C, frame = 3, 3 * U
+    T = 2 * frame
+    seed = synth.config_seed(4)
+    freqs = np.array([800.0, 611.71875, 400.390625])
+    gains = synth.gains(seed, C, flagged_frac=0.10)
+    b = synth.noise_bytes(seed, C, T)
+    b, _ = synth.saturate_bursts(b, seed)
+    plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, zero_pad=NP, upchan_len=U, n_time=T)
+    hb = b.numpy()
+    cells = [(c, R) for c in range(C) for R in range(2)]
+    worst, frac = compare_cells(orc, plan, b.cuda(), lambda c, R: hb[c, frame * R:frame * (R + 1)], freqs,
+                                gains, cells, NP, U)
+    print(f"NP={NP} U={U}: worst rel err {worst:.2e}, u8 diff frac {frac:.2e}")
+
+
+def test_degenerate_inputs(bf, orc):
+    plan = bf.plan_create_ex(1, freq_mhz=[612.5], n_time=384)
+    z = torch.full((1, 384, 2048), 0x88, dtype=torch.uint8, device="cuda")
+    assert torch.all(plan.execute_f32(z) == 0)
+    assert torch.all(plan.execute(z) == 128)
+    # all gains zero
+    g0 = np.zeros((1, 2048, 2), dtype=np.float32)
+    plan0 = bf.plan_create_ex(1, freq_mhz=[612.5], gains=g0, n_time=384)
+    nb = synth.noise_bytes(3, 1, 384).cuda()
+    assert torch.all(plan0.execute(nb) == 128)
+    # saturation of the quantiser: every sample at +7+7i on every input -> huge zenith power -> 255
+    s = torch.full((1, 384, 2048), 0xFF, dtype=torch.uint8, device="cuda")
+    q = plan.execute(s)
+    assert int(q.max()) == 255 and int(q.min()) == 128
+
+
+def test_execute_host_matches_device(bf):
+    T = 768
+    plan = bf.plan_create_ex(2, n_time=T)
+    b = synth.noise_bytes(11, 2, T)
+    ref = plan.execute(b.cuda()).cpu()
+    out = plan.execute_host(b.pin_memory())
+    assert torch.equal(ref, out.reshape(ref.shape))
+
+
+def test_cfg1_full_size_sampled(bf, orc):
+    """BASELINE config 1 at full size, in the launch configuration bench.py times; the oracle checks a
+    seeded sample of cells (cells are independent)."""
+    cfg = synth.CONFIGS[1]
+    C, T = cfg["n_coarse"], cfg["n_time"]
+    seed = synth.config_seed(1)
+    freqs = synth.config_freqs(1)
+    gains = synth.gains(seed, C, flagged_frac=cfg["flagged"])
+    d_in = synth.noise_bytes(seed, C, T, device="cuda")
+    plan = bf.plan_create(C, gains=gains)          # north-star form: default freqs, n_time 49152
+    rng = np.random.default_rng(seed)
+    cells = [(0, 0), (C - 1, T // 384 - 1)] + [(int(rng.integers(C)), int(rng.integers(T // 384))) for _ in range(10)]
+
+    def host_bytes(c, R):
+        blk = d_in[c, 384 * R:384 * (R + 1)].cpu().numpy()
+        # the generator is counter-based: the same block drawn on the CPU must be identical
+        if R == 0:
+            assert np.array_equal(blk, synth.noise_bytes(seed, 1, 384, chan0=c, time0=0, n_time_total=T).numpy()[0])
+        return blk
+
+    worst, frac = compare_cells(orc, plan, d_in, host_bytes, freqs, gains, cells, 512, 128)
+    print(f"cfg1: worst rel err {worst:.2e}, u8 diff frac {frac:.2e}")
