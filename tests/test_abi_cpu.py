@@ -71,5 +71,6 @@ def test_product_does_not_import_oracle():
     for fn in os.listdir(os.path.join(ROOT, "oracle")):
         if fn.endswith((".py", ".c")):
             src = open(os.path.join(ROOT, "oracle", fn)).read()
-            code = "\n".join(l for l in src.splitlines() if l.strip().startswith(("import ", "from ", "#include")))
+            code = "\n".join(l for l in src.splitlines()
+                             if re.match(r"\s*(import\s+[\w.]+(\s+as\s+\w+)?\s*$|from\s+[\w.]+\s+import\s|#include)", l))
             assert "paper_1702_04728_b200" not in code and "csrc" not in code and "chime_bf.h" not in code
