@@ -1,0 +1,288 @@
+"""bench.py -- one JSON line per run (contract in DESIGN.md "Measurement").
+
+A "step" is one pass of the whole hot path (a1-a10, one chime_bf_execute) over one batch of
+synthetic CHIME-shaped baseband: BASELINE.json configs[1] (4 coarse channels x 49152 samples x 2048
+inputs = 403 MB in, 8.4 MB out) per GPU.  metric = input baseband GB/s (and, beside it, the number of
+coarse channels that rate sustains in real time, 1 channel = 0.8 GB/s).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W]          CUDA arm
+  python bench.py --impl reference ...                         oracle arm (CPU, bounded sample)
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "input baseband GB/s and coarse channels sustained in real time per B200"
+UNIT = "GB/s"
+BYTES_PER_CHAN_SAMPLE = 2048.0
+REALTIME_SAMPLES_PER_S = 390625.0                 # 1 / 2.56 us  (Table 1)
+GBS_PER_CHANNEL = BYTES_PER_CHAN_SAMPLE * REALTIME_SAMPLES_PER_S / 1e9   # 0.8 GB/s
+# Nominal flops per (channel, sample): FFTs only / everything.
+FFT_FLOPS = 256000.0
+ALL_FLOPS = 342016.0
+# FP32 peak: 148 SMs x 128 lanes x 2 flop x sm clock (DESIGN.md derives it; clock from MEASURED_PEAKS).
+N_SM, LANES = 148, 128
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            p = [x.strip() for x in r.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(n_cells, seed_cfg=1):
+    """Times the oracle, as it stands, on n_cells output cells (1 cell = 1 channel x 384 samples) of the
+    configs[1] workload.  Returns (seconds, chan_samples, cores)."""
+    import numpy as np
+    import oracle
+    import synth
+    oracle.build()
+    cfg = synth.CONFIGS[seed_cfg]
+    C, T = cfg["n_coarse"], cfg["n_time"]
+    seed = synth.config_seed(seed_cfg)
+    freqs = synth.config_freqs(seed_cfg)
+    gains = synth.gains(seed, C, flagged_frac=cfg["flagged"])
+    rng = np.random.default_rng(seed)
+    cells = [(int(rng.integers(C)), int(rng.integers(T // 384))) for _ in range(n_cells)]
+    blocks = [synth.noise_bytes(seed, 1, 384, chan0=c, time0=384 * R, n_time_total=T).numpy()[0]
+              for (c, R) in cells]
+    t0 = time.perf_counter()
+    for (c, R), blk in zip(cells, blocks):
+        I, _ = oracle.cell(blk, float(freqs[c]), gains=gains[c])
+        oracle.quantize(I)
+    dt = time.perf_counter() - t0
+    return dt, n_cells * 384, oracle.max_threads()
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, each step a bounded sample (4 cells)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cells_per_step = 4
+    for _ in range(args.warmup):
+        oracle_sample(1)
+    t_tot, cs_tot, cores = 0.0, 0, 1
+    for _ in range(args.steps):
+        dt, cs, cores = oracle_sample(cells_per_step)
+        t_tot += dt
+        cs_tot += cs
+    gbs = cs_tot * BYTES_PER_CHAN_SAMPLE / t_tot / 1e9
+    sample = f"{cells_per_step} cells (channel x 384-sample frame) of configs[1] per step, oracle as it stands"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "channels_realtime": gbs / GBS_PER_CHANNEL,
+        "config": {"workload": "configs[1] single node load: 4 coarse channels x 49152 samples x 2048 inputs "
+                               "(bounded sample of its output cells)"},
+        "cpu_baseline": {"value": gbs, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gbs, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def run_cuda(args):
+    import numpy as np
+    import torch
+
+    import paper_1702_04728_b200 as bf
+    import synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    bf.load_library()
+
+    # ---- workload: configs[1], channels sharded over ranks (weak scaling: 4 channels per GPU) ----
+    cfg = synth.CONFIGS[1]
+    C, T = cfg["n_coarse"], cfg["n_time"]
+    seed = synth.config_seed(1)
+    chan0 = rank * C
+    freqs = synth.chime_freqs_mhz(C, 1, k0=chan0)
+    gains = synth.gains(seed + 1000 * rank, C, flagged_frac=cfg["flagged"])
+    plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, zero_pad=512, upchan_len=128, n_time=T)
+    d_in = synth.noise_bytes(seed, C, T, device="cuda", chan0=chan0)
+    d_out = torch.empty(plan.out_shape, dtype=torch.uint8, device="cuda")
+    h_in = d_in.cpu().pin_memory()
+    h_out = torch.empty(plan.out_shape, dtype=torch.uint8).pin_memory()
+    in_bytes, out_bytes = plan.in_bytes, plan.out_elems
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+
+    # ---- device-resident: K steps, per-step CUDA events on the launching stream ----
+    for _ in range(max(args.warmup, 3)):
+        plan.execute(d_in, d_out, stream=stream)
+    barrier()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for a, b in evs:
+        a.record(stream)
+        plan.execute(d_in, d_out, stream=stream)
+        b.record(stream)
+    e1.record(stream)
+    barrier()
+    total_ms = e0.elapsed_time(e1)
+    kern_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+
+    # ---- end to end through the C-ABI with HOST buffers (H2D + kernel + D2H inside the call) ----
+    n_e2e = max(2, min(args.steps, 5))
+    plan.execute_host(h_in, h_out, stream=stream)
+    barrier()
+    t0 = time.perf_counter()
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g0.record(stream)
+    for _ in range(n_e2e):
+        plan.execute_host(h_in, h_out, stream=stream)
+    g1.record(stream)
+    barrier()
+    e2e_ms = g0.elapsed_time(g1)
+    clocks = sampler.stop() if rank == 0 else None
+    assert torch.equal(h_out, d_out.cpu()), "host path and device path disagree"
+
+    if dist is not None:
+        t = torch.tensor([total_ms, kern_ms, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, kern_ms, e2e_ms = [float(x) for x in t.tolist()]
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    gbs = world * args.steps * in_bytes / (total_ms * 1e-3) / 1e9
+    e2e_gbs = world * n_e2e * in_bytes / (e2e_ms * 1e-3) / 1e9
+    peaks, peak_kind = measured_peaks()
+    sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    fp32_peak = N_SM * LANES * 2 * sm_mhz * 1e6 / 1e12
+    chan_samples = C * T
+    ach = FFT_FLOPS * chan_samples / (kern_ms * 1e-3) / 1e12
+    hbm_peak = float(peaks["hbm_gbs"])
+    hbm_ach = (in_bytes + out_bytes) / (kern_ms * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "channels_realtime": gbs / GBS_PER_CHANNEL,
+        "realtime_fraction_full_band": gbs / (1024 * GBS_PER_CHANNEL),
+        "config": {"workload": "configs[1] single node load per GPU: 4 coarse channels x 49152 samples x "
+                               "2048 inputs, zero_pad 512, upchan 128, random gains, 2% flagged",
+                   "in_bytes_per_step": in_bytes, "out_bytes_per_step": out_bytes,
+                   "l2": "input (403 MB) larger than L2 (126 MB); no flush needed",
+                   "parallelism": f"channel-sharded x{world}, no collective"},
+        "roofline": {"bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s",
+                     "frac": ach / fp32_peak, "traffic": None,
+                     "kernel": "beamform_fused_kernel<2,4>", "kernel_ms": kern_ms,
+                     "flops_per_chan_sample": FFT_FLOPS,
+                     "note": f"FP32 peak = 148 SM x 128 lanes x 2 x {sm_mhz:.0f} MHz ({peak_kind} sm_max_mhz); "
+                             "nominal FFT flops (5 n log2 n) per BASELINE north_star",
+                     "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
+                             "peak_kind": peak_kind}},
+        "e2e": {"value": e2e_gbs, "unit": UNIT, "h2d_bytes_per_step": in_bytes,
+                "d2h_bytes_per_step": out_bytes, "steps": n_e2e},
+        "gpu_launches": args.steps * plan.launches_per_execute,
+        "clocks": clocks,
+    }
+    if not args.no_cpu_baseline and world >= 1:
+        dt, cs, cores = oracle_sample(32)
+        v = cs * BYTES_PER_CHAN_SAMPLE / dt / 1e9
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": "32 output cells (channel x 384 samples) of configs[1], "
+                                          f"{dt:.1f} s of oracle time", "channels_realtime": v / GBS_PER_CHANNEL}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    return run_reference(args) if args.impl == "reference" else run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
