@@ -8,10 +8,12 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
 #include "beamform_kernel.cuh"
+#include "beamform_mma_kernel.cuh"
 
 namespace {
 
@@ -39,6 +41,8 @@ struct chime_bf_plan {
     int16_t *d_slot_of_m = nullptr;
     float2 *d_tw_np = nullptr;
     float2 *d_tw_u = nullptr;
+    uint2 *d_bfrag = nullptr;  // tensor-core B fragments of the folded weights (zero_pad 512, upchan 128 path)
+    bool use_mma = false;
     // staging for execute_host
     uint8_t *d_stage_in = nullptr;
     uint8_t *d_stage_out = nullptr;
@@ -121,6 +125,36 @@ bool build_tables(chime_bf_plan *pl, const chime_bf_params &p, double fref, doub
             }
         }
     }
+    // Tensor-core path (beamform_mma_kernel.cuh): per (c, pol, beam pair ep, feed n) the 8 x 8 real
+    // embedding of the 4 cyl x 2 beam complex weights, as mma.m16n8k8 B fragments (lane = 4 g + tq holds
+    // rows k = 2 tq, 2 tq + 1 of column g), scaled by 2^9 and split hi + lo in fp16.  Columns 4..7 are
+    // zero, so only lanes 0..15 are stored.
+    std::vector<uint2> bfrag;
+    if (pl->use_mma) {
+        bfrag.resize((size_t)C * 2 * 2 * 256 * 16);
+        auto split = [](float v, uint16_t &hi, uint16_t &lo) {
+            const __half h = __float2half_rn(v);
+            const __half l = __float2half_rn(v - __half2float(h));
+            memcpy(&hi, &h, 2);
+            memcpy(&lo, &l, 2);
+        };
+        for (int c = 0; c < C; ++c)
+            for (int pol = 0; pol < 2; ++pol)
+                for (int ep = 0; ep < 2; ++ep)
+                    for (int n = 0; n < 256; ++n)
+                        for (int lane = 0; lane < 16; ++lane) {
+                            const int g = lane >> 2, cyl = lane & 3, e = 2 * ep + (g >> 1), ro = g & 1;
+                            const float2 w = wp[((((size_t)c * 2 + pol) * 4 + e) * 4 + cyl) * 256 + n];
+                            // output re: k=(cyl,re)-> wr, k=(cyl,im)-> -wi ; output im: wi, wr
+                            const float k0 = 512.0f * (ro == 0 ? w.x : w.y);
+                            const float k1 = 512.0f * (ro == 0 ? -w.y : w.x);
+                            uint16_t h0, l0, h1, l1;
+                            split(k0, h0, l0);
+                            split(k1, h1, l1);
+                            bfrag[((((size_t)c * 2 + pol) * 2 + ep) * 256 + n) * 16 + lane] =
+                                make_uint2((uint32_t)h0 | ((uint32_t)h1 << 16), (uint32_t)l0 | ((uint32_t)l1 << 16));
+                        }
+    }
     std::vector<float2> tw_np(NP), tw_u(U);
     for (int k = 0; k < NP; ++k) {
         const double a = -2.0 * kPi * (double)k / (double)NP;
@@ -129,6 +163,17 @@ bool build_tables(chime_bf_plan *pl, const chime_bf_params &p, double fref, doub
     for (int k = 0; k < U; ++k) {
         const double a = -2.0 * kPi * (double)k / (double)U;
         tw_u[k] = make_float2((float)std::cos(a), (float)std::sin(a));
+    }
+    if (pl->use_mma) {
+        std::vector<float2> tw128(128);
+        for (int k = 0; k < 128; ++k) {
+            const double a = -2.0 * kPi * (double)k / 128.0;
+            tw128[k] = make_float2((float)std::cos(a), (float)std::sin(a));
+        }
+        CUDA_TRY(cudaMemcpyToSymbol(chime2::c_tw128, tw128.data(), sizeof(float2) * 128));
+        CUDA_TRY(cudaFuncSetAttribute(chime2::beamform_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      chime2::kSmemBytes));
+        if (!upload(&pl->d_bfrag, bfrag)) return false;
     }
     return upload(&pl->d_wp, wp) && upload(&pl->d_slot, slot) && upload(&pl->d_slot_of_m, slot_of_m) &&
            upload(&pl->d_tw_np, tw_np) && upload(&pl->d_tw_u, tw_u);
@@ -171,8 +216,31 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
     kp.norm = pl->norm;
     kp.qscale = pl->norm * pl->scale;
     kp.qoffset = pl->offset;
-    const int n_cta = pl->C * pl->R * 4;
     cudaStream_t st = (cudaStream_t)stream;
+    if (pl->use_mma) {
+        chime2::Params mp;
+        mp.in = in;
+        mp.out_u8 = out_u8;
+        mp.out_f32 = out_f32;
+        mp.bfrag = pl->d_bfrag;
+        mp.slot = pl->d_slot;
+        mp.slot_of_m = pl->d_slot_of_m;
+        mp.tw_np = pl->d_tw_np;
+        mp.n_time = pl->T;
+        mp.n_frames = pl->R;
+        mp.norm = pl->norm;
+        mp.qscale = pl->norm * pl->scale;
+        mp.qoffset = pl->offset;
+        mp.dbg = getenv("CHIME_BF_DBG") ? (float *)strtoull(getenv("CHIME_BF_DBG"), nullptr, 0) : nullptr;
+        chime2::beamform_mma_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
+        const cudaError_t e2 = cudaGetLastError();
+        if (e2 != cudaSuccess) {
+            set_err("kernel launch failed: %s", cudaGetErrorString(e2));
+            return CHIME_BF_E_CUDA;
+        }
+        return CHIME_BF_OK;
+    }
+    const int n_cta = pl->C * pl->R * 4;
     cudaError_t e = cudaErrorInvalidValue;
     const int P = pl->NP / 256, RAD = pl->U / 32;
     if (P == 1 && RAD == 4) e = launch<1, 4>(kp, n_cta, st);
@@ -232,6 +300,7 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     pl->scale = p.scale > 0.f ? p.scale : 1.0f / 64.0f;
     pl->offset = p.scale > 0.f ? p.offset : 128.0f;
     pl->norm = (float)(1.0 / (256.0 * 4.0 * (double)p.upchan_len));
+    pl->use_mma = (p.zero_pad == 512 && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
     cudaGetDevice(&pl->device);
     const double fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
     const double d_feed = p.feed_spacing_m > 0 ? p.feed_spacing_m : 0.3048;
@@ -336,6 +405,7 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_slot_of_m);
     cudaFree(pl->d_tw_np);
     cudaFree(pl->d_tw_u);
+    cudaFree(pl->d_bfrag);
     cudaFree(pl->d_stage_in);
     cudaFree(pl->d_stage_out);
     delete pl;
