@@ -52,7 +52,6 @@ struct Params {
     int n_time;
     int n_frames;
     float norm, qscale, qoffset;
-    float *dbg;  // TEMP debug dump
 };
 
 __constant__ float2 c_tw128[128];  // exp(-2 pi i k / 128), uploaded at plan creation
@@ -139,19 +138,25 @@ __device__ __forceinline__ void phase_a(const unsigned char *raw, float2 *tile, 
     const bool stores = tq < 2;             // C columns 0..3 = (e' = tq, re/im)
     const int r0 = g * 2 + tq;              // tile row of (u' = g, e' = tq); u' = g + 8 -> r0 + 16
 
-#pragma unroll 1
+    // raw address of (u' = g + 8 hr, tap k): piece p = 4 (g + 8 hr + 16 k) + tq, and p & 15 = 4 (g & 3) + tq
+    // for every (hr, k), so the swizzled unit is a per-thread constant and (hr, k) are immediate offsets.
+    const int pz = 4 * (g & 3) + tq;
+    const unsigned char *raw_t = raw + (4 * g + tq) * 256;
+    // tile address of (row r0 [+16], feed n): n >> 1 = 8 warp + 4 hh + i / 2, so the swizzled 16-byte chunk is
+    // ((4 hh + i / 2) ^ (r0 & 7)); byte offset = row + line(n >> 4 = warp) * 128 + chunk * 16.
+    unsigned char *tile_t = reinterpret_cast<unsigned char *>(tile) + r0 * 2048 + warp * 128;
+    const int rx16 = (r0 & 7) << 4;
+
+#pragma unroll
     for (int hh = 0; hh < 2; ++hh) {        // 8 feeds at a time
         uint32_t aE[2][8], aO[2][8];
+        const unsigned char *raw_h = raw_t + (((2 * warp + hh) ^ pz) << 3);
 #pragma unroll
         for (int hr = 0; hr < 2; ++hr) {
-            const int u = g + 8 * hr;
             uint2 q[8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                const int p = 4 * (u + 16 * k) + tq;
-                const int unit = (2 * warp + hh) ^ (p & 15);
-                q[k] = *reinterpret_cast<const uint2 *>(raw + p * 256 + unit * 8);
-            }
+            for (int k = 0; k < 8; ++k)
+                q[k] = *reinterpret_cast<const uint2 *>(raw_h + (32 * hr + 64 * k) * 256);
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
                 uint32_t er, ei, orr, oi, pr, pi;
@@ -201,9 +206,9 @@ __device__ __forceinline__ void phase_a(const unsigned char *raw, float2 *tile, 
                 }
             }
             if (stores) {
-                const int n = n0 + i;  // even
-                *reinterpret_cast<float4 *>(tile + tile_idx(r0, n)) = make_float4(z[0][0], z[0][1], z[1][0], z[1][1]);
-                *reinterpret_cast<float4 *>(tile + tile_idx(r0 + 16, n)) = make_float4(z[0][2], z[0][3], z[1][2], z[1][3]);
+                unsigned char *dst = tile_t + (rx16 ^ ((4 * hh + i / 2) << 4));
+                *reinterpret_cast<float4 *>(dst) = make_float4(z[0][0], z[0][1], z[1][0], z[1][1]);
+                *reinterpret_cast<float4 *>(dst + 16 * 2048) = make_float4(z[0][2], z[0][3], z[1][2], z[1][3]);
             }
         }
     }
@@ -213,13 +218,20 @@ __device__ __forceinline__ void phase_a(const unsigned char *raw, float2 *tile, 
 // Half-warp h computes the bins of parity h: FFT-256 of a[n] W_512^{h n}.  twc[j2] = W_512^{l (2 j2 + h)}
 // merges the inter-stage twiddle W_256^{l j2} with the lane part W_512^{h l} of the pre-twiddle; the
 // rest of the pre-twiddle, W_32^{h k}, has compile-time arguments.
-__device__ __forceinline__ void phase_b_row(float2 *tile, float2 *exw, const int16_t *s_slot, const int r,
-                                            const int h, const int l, const float2 (&twc)[16]) {
-    const int rx = r & 7;
+// All shared-memory addresses are (per-thread constant) XOR (immediate) + immediate:
+//   row read      row + 128 k + rd,            rd = (((l>>1) ^ rx) << 4) | ((l&1) << 3)
+//   exch write    ex + 128 j2 + (wr ^ ((j2&7) << 4)),  wr = (((l>>1) ^ x) << 4) | ((l&1) << 3)
+//   exch read     ex + (er ^ (i << 4)),        er = 128 l | (((l&7) ^ x) << 4)
+// with rx = r & 7 (the row's swizzle; identical for the warp's two rows r and r + 16), x = rx (even half,
+// exchanging through the row) or 0 (odd half, private buffer).
+// s_sel[(16 h + l) * 16 + i] = slot of bin 2 (16 bitrev(i) + l) + h, or -1; slot -> byte (slot ^ (rx << 1)) * 8.
+__device__ __forceinline__ void phase_b_row(unsigned char *S, const int rowofs, const int exofs, const int h,
+                                            const int rd, const int wr, const int er, const int rx2,
+                                            const uint4 sel0, const uint4 sel1, const float2 (&twc)[16]) {
     float2 a[16];
+    const int ra = rowofs + rd;
 #pragma unroll
-    for (int k = 0; k < 16; ++k)
-        a[k] = tile[r * 256 + 16 * k + ((((l >> 1) ^ rx)) << 1) + (l & 1)];
+    for (int k = 0; k < 16; ++k) a[k] = *reinterpret_cast<const float2 *>(S + (ra + 128 * k));
     if (h) {
         a[1] = chime::twiddle64<2>(a[1]);   a[2] = chime::twiddle64<4>(a[2]);   a[3] = chime::twiddle64<6>(a[3]);
         a[4] = chime::twiddle64<8>(a[4]);   a[5] = chime::twiddle64<10>(a[5]);  a[6] = chime::twiddle64<12>(a[6]);
@@ -229,45 +241,51 @@ __device__ __forceinline__ void phase_b_row(float2 *tile, float2 *exw, const int
     }
     fft_dif<16>(a);
     __syncwarp();  // every lane has read the row before the even half overwrites it
-    // exchange: element (j2, l) -> line j2, 16-byte chunk (l>>1) ^ (j2&7) ^ x, x = row swizzle (even half) or 0
-    float2 *ex = h ? exw : tile + r * 256;
-    const int x = h ? 0 : rx;
+    const int wa = exofs + wr, ea = exofs + er;
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         const int j2 = bitrev(i, 4);
-        ex[16 * j2 + ((((l >> 1) ^ (j2 & 7) ^ x)) << 1) + (l & 1)] = cmul(a[i], twc[j2]);
+        *reinterpret_cast<float2 *>(S + ((wa ^ ((j2 & 7) << 4)) + 128 * j2)) = cmul(a[i], twc[j2]);
     }
     __syncwarp();
     float2 b[16];
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
-        const float4 v = *reinterpret_cast<const float4 *>(ex + 16 * l + ((i ^ (l & 7) ^ x) << 1));
+        const float4 v = *reinterpret_cast<const float4 *>(S + (ea ^ (i << 4)));
         b[2 * i] = make_float2(v.x, v.y);
         b[2 * i + 1] = make_float2(v.z, v.w);
     }
     fft_dif<16>(b);
     __syncwarp();  // all exchange reads done before slots are written into the row
+    const uint32_t sw[8] = {sel0.x, sel0.y, sel0.z, sel0.w, sel1.x, sel1.y, sel1.z, sel1.w};
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
-        const int j1 = bitrev(i, 4);
-        const int s = s_slot[2 * (16 * j1 + l) + h];
-        if (s >= 0) tile[r * 256 + (s & ~15) + ((((s >> 1) & 7) ^ rx) << 1) + (s & 1)] = b[i];
+        const int s = (int)(int16_t)((i & 1) ? (sw[i >> 1] >> 16) : (sw[i >> 1] & 0xFFFFu));
+        if (s >= 0) *reinterpret_cast<float2 *>(S + (rowofs + ((s ^ rx2) << 3))) = b[i];
+    }
+}
+
+// a[u] *= exp(-2 pi i RHO u / 128), u = U..15: even RHO u are compile-time twiddle64 arguments, odd ones
+// come from the 128-point table in constant memory (compile-time index -> constant-bank operand).
+template <int RHO, int U>
+__device__ __forceinline__ void time_pretwiddle(float2 (&a)[16]) {
+    if constexpr (U < 16) {
+        if constexpr (((RHO * U) & 1) == 0) a[U] = chime::twiddle64<((RHO * U) / 2) & 63>(a[U]);
+        else a[U] = cmul(a[U], c_tw128[(RHO * U) & 127]);
+        time_pretwiddle<RHO, U + 1>(a);
     }
 }
 
 // ---- phase C: thread <-> (e', slot): 16-point time FFT, detect, accumulate ---------------------------
-__device__ __forceinline__ void phase_c(const float2 *tile, const int rho, const int ep, const int s,
-                                        float (&acc)[16]) {
+// col = byte offset of (row e', slot) with the row-independent part of the swizzle applied; row 2 u + e'
+// adds 4096 u and XORs the 16-byte chunk index with 2 (u & 3).
+template <int RHO>
+__device__ __forceinline__ void phase_c(const unsigned char *S, const int col, float (&acc)[16]) {
     float2 a[16];
 #pragma unroll
-    for (int u = 0; u < 16; ++u) {
-        const int r = 2 * u + ep;
-        a[u] = tile[r * 256 + (s & ~15) + ((((s >> 1) & 7) ^ (r & 7)) << 1) + (s & 1)];
-    }
-    if (rho != 0) {
-#pragma unroll
-        for (int u = 1; u < 16; ++u) a[u] = cmul(a[u], c_tw128[(rho * u) & 127]);
-    }
+    for (int u = 0; u < 16; ++u)
+        a[u] = *reinterpret_cast<const float2 *>(S + ((col ^ ((2 * (u & 3)) << 4)) + 4096 * u));
+    if constexpr (RHO != 0) time_pretwiddle<RHO, 1>(a);
     fft_dif<16>(a);
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
@@ -276,13 +294,19 @@ __device__ __forceinline__ void phase_c(const float2 *tile, const int rho, const
     }
 }
 
+template <int RHO>
+__device__ __forceinline__ void phase_a_rho(const unsigned char *raw, float2 *tile, const uint2 *bf, int warp, int lane) {
+    phase_a<RHO>(raw, tile, bf, warp, lane);
+}
+
 __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params prm) {
-    extern __shared__ __align__(16) unsigned char smem[];
+    extern __shared__ __align__(1024) unsigned char smem[];
+    unsigned char *const S = smem;
     unsigned char *raw = smem;                                                   // 128 KiB
-    float2 *tile = reinterpret_cast<float2 *>(smem + kRawBytes);                 // [32][256]
-    float2 *exch = reinterpret_cast<float2 *>(smem + kRawBytes + kTileBytes);    // [16 warps][256]
-    int16_t *s_slot = reinterpret_cast<int16_t *>(smem + kRawBytes + kTileBytes + kExchBytes);  // [512]
-    int16_t *s_slot_of_m = s_slot + 512;                                         // [256]
+    float2 *tile = reinterpret_cast<float2 *>(smem + kRawBytes);                 // [32][256], swizzled
+    constexpr int kTileOfs = kRawBytes, kExchOfs = kRawBytes + kTileBytes;
+    int16_t *s_sel = reinterpret_cast<int16_t *>(smem + kRawBytes + kTileBytes + kExchBytes);  // [32][16]
+    int16_t *s_slot_of_m = s_sel + 512;                                          // [256]
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ep = blockIdx.x & 1;
@@ -290,11 +314,20 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
     const int Rf = cell % prm.n_frames;
     const int c = cell / prm.n_frames;
 
-    s_slot[tid] = prm.slot[(size_t)c * 512 + tid];
+    {   // s_sel[(16 h + l) * 16 + i] = slot of bin 2 (16 bitrev(i) + l) + h
+        const int i = tid & 15, hl = tid >> 4;
+        s_sel[tid] = prm.slot[(size_t)c * 512 + 2 * (16 * bitrev(i, 4) + (hl & 15)) + (hl >> 4)];
+    }
     if (tid < 256) s_slot_of_m[tid] = prm.slot_of_m[(size_t)c * 256 + tid];
 
-    // phase B lane constants
+    // phase B per-thread constants (rows warp and warp + 16 share the swizzle rx = warp & 7)
     const int h = lane >> 4, l = lane & 15;
+    const int rx = warp & 7, xx = h ? 0 : rx;
+    const int rd = (((l >> 1) ^ rx) << 4) | ((l & 1) << 3);
+    const int wr = (((l >> 1) ^ xx) << 4) | ((l & 1) << 3);
+    const int er = (128 * l) | (((l & 7) ^ xx) << 4);
+    const int row0 = kTileOfs + warp * 2048, row1 = row0 + 16 * 2048;
+    const int exw = kExchOfs + warp * 2048;
     float2 twc[16];
 #pragma unroll
     for (int j2 = 0; j2 < 16; ++j2) twc[j2] = __ldg(prm.tw_np + ((l * (2 * j2 + h)) & 511));
@@ -303,14 +336,16 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
 #pragma unroll
     for (int g = 0; g < 16; ++g) acc[g] = 0.f;
 
-    const int e1 = tid >> 8, sl = tid & 255;  // phase C mapping
+    // phase C per-thread constants
+    const int e1 = tid >> 8, sl = tid & 255;
+    const int col = kTileOfs + e1 * 2048 + (sl >> 4) * 128 + ((((sl >> 1) & 7) ^ e1) << 4) + (sl & 1) * 8;
     const uint8_t *in_c = prm.in + (size_t)c * prm.n_time * 2048;
 
 #pragma unroll 1
     for (int blk = 0; blk < 6; ++blk) {
         const int r3 = blk >> 1, pol = blk & 1;
         const int t0 = (Rf * 3 + r3) * 128;
-        __syncthreads();  // previous block's phase A reads of raw are long done; also covers s_slot init
+        __syncthreads();  // covers the table initialisation; raw is free (last phase A ended 2 barriers ago)
         // ---- stage the raw block: 8192 16-byte chunks, 16 per thread, coalesced 512 B per warp ----
 #pragma unroll
         for (int j0 = 0; j0 < 16; j0 += 4) {
@@ -337,28 +372,33 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
 #pragma unroll 1
         for (int rho = 0; rho < 8; ++rho) {
             switch (rho) {
-                case 0: phase_a<0>(raw, tile, bf, warp, lane); break;
-                case 1: phase_a<1>(raw, tile, bf, warp, lane); break;
-                case 2: phase_a<2>(raw, tile, bf, warp, lane); break;
-                case 3: phase_a<3>(raw, tile, bf, warp, lane); break;
-                case 4: phase_a<4>(raw, tile, bf, warp, lane); break;
-                case 5: phase_a<5>(raw, tile, bf, warp, lane); break;
-                case 6: phase_a<6>(raw, tile, bf, warp, lane); break;
-                default: phase_a<7>(raw, tile, bf, warp, lane); break;
+                case 0: phase_a_rho<0>(raw, tile, bf, warp, lane); break;
+                case 1: phase_a_rho<1>(raw, tile, bf, warp, lane); break;
+                case 2: phase_a_rho<2>(raw, tile, bf, warp, lane); break;
+                case 3: phase_a_rho<3>(raw, tile, bf, warp, lane); break;
+                case 4: phase_a_rho<4>(raw, tile, bf, warp, lane); break;
+                case 5: phase_a_rho<5>(raw, tile, bf, warp, lane); break;
+                case 6: phase_a_rho<6>(raw, tile, bf, warp, lane); break;
+                default: phase_a_rho<7>(raw, tile, bf, warp, lane); break;
             }
             __syncthreads();
-            if (prm.dbg && blockIdx.x == 0 && blk == 0 && rho == 1) {
-                for (int i = tid; i < 32 * 256; i += kThreads) { prm.dbg[2 * i] = tile[i].x; prm.dbg[2 * i + 1] = tile[i].y; }
-                __syncthreads();
+            {
+                const uint4 sel0 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16);
+                const uint4 sel1 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16 + 8);
+                phase_b_row(S, row0, h ? exw : row0, h, rd, wr, er, rx << 1, sel0, sel1, twc);
+                phase_b_row(S, row1, h ? exw : row1, h, rd, wr, er, rx << 1, sel0, sel1, twc);
             }
-            phase_b_row(tile, exch + warp * 256, s_slot, warp, h, l, twc);
-            phase_b_row(tile, exch + warp * 256, s_slot, warp + 16, h, l, twc);
             __syncthreads();
-            if (prm.dbg && blockIdx.x == 0 && blk == 0 && rho == 1) {
-                for (int i = tid; i < 32 * 256; i += kThreads) { prm.dbg[16384 + 2 * i] = tile[i].x; prm.dbg[16384 + 2 * i + 1] = tile[i].y; }
-                __syncthreads();
+            switch (rho) {
+                case 0: phase_c<0>(S, col, acc); break;
+                case 1: phase_c<1>(S, col, acc); break;
+                case 2: phase_c<2>(S, col, acc); break;
+                case 3: phase_c<3>(S, col, acc); break;
+                case 4: phase_c<4>(S, col, acc); break;
+                case 5: phase_c<5>(S, col, acc); break;
+                case 6: phase_c<6>(S, col, acc); break;
+                default: phase_c<7>(S, col, acc); break;
             }
-            phase_c(tile, rho, e1, sl, acc);
             __syncthreads();
         }
     }

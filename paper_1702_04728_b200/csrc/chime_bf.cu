@@ -231,7 +231,6 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         mp.norm = pl->norm;
         mp.qscale = pl->norm * pl->scale;
         mp.qoffset = pl->offset;
-        mp.dbg = getenv("CHIME_BF_DBG") ? (float *)strtoull(getenv("CHIME_BF_DBG"), nullptr, 0) : nullptr;
         chime2::beamform_mma_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
         const cudaError_t e2 = cudaGetLastError();
         if (e2 != cudaSuccess) {
