@@ -167,7 +167,8 @@ def run_cuda(args):
     cfg = synth.CONFIGS[1]
     C, T = cfg["n_coarse"], cfg["n_time"]
     seed = synth.config_seed(1)
-    chan0 = rank * C
+    from paper_1702_04728_b200.sharding import weak_scaling_shard
+    chan0, _ = weak_scaling_shard(C, rank)
     freqs = synth.chime_freqs_mhz(C, 1, k0=chan0)
     gains = synth.gains(seed + 1000 * rank, C, flagged_frac=cfg["flagged"])
     plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, zero_pad=512, upchan_len=128, n_time=T)
@@ -237,6 +238,13 @@ def run_cuda(args):
     ach = FFT_FLOPS * chan_samples / (kern_ms * 1e-3) / 1e12
     hbm_peak = float(peaks["hbm_gbs"])
     hbm_ach = (in_bytes + out_bytes) / (kern_ms * 1e-3) / 1e9
+    traffic, traffic_src = None, None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            tj = json.load(f)
+        traffic, traffic_src = float(tj["dram_bytes_per_launch"]), tj["source"]
+    except Exception:
+        pass
     line = {
         "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -249,8 +257,10 @@ def run_cuda(args):
                    "l2": "input (403 MB) larger than L2 (126 MB); no flush needed",
                    "parallelism": f"channel-sharded x{world}, no collective"},
         "roofline": {"bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s",
-                     "frac": ach / fp32_peak, "traffic": None,
-                     "kernel": "beamform_fused_kernel<2,4>", "kernel_ms": kern_ms,
+                     "frac": ach / fp32_peak, "traffic": traffic,
+                     "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
+                     "traffic_source": traffic_src, "algorithmic_bytes": in_bytes + out_bytes,
+                     "kernel": "chime2::beamform_mma_kernel", "kernel_ms": kern_ms,
                      "flops_per_chan_sample": FFT_FLOPS,
                      "note": f"FP32 peak = 148 SM x 128 lanes x 2 x {sm_mhz:.0f} MHz ({peak_kind} sm_max_mhz); "
                              "nominal FFT flops (5 n log2 n) per BASELINE north_star",
