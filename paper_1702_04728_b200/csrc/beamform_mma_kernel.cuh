@@ -39,7 +39,8 @@ constexpr int kTileRows = kRowsT * 2;            // x 2 beams of the pair
 constexpr int kRawBytes = 128 * 4 * 256;         // one (block, pol): 128 KiB
 constexpr int kTileBytes = kTileRows * 256 * 8;  // 64 KiB
 constexpr int kExchBytes = kWarps * 256 * 8;     // 32 KiB
-constexpr int kSmemBytes = kRawBytes + kTileBytes + kExchBytes + 512 * 2 + 256 * 2;
+constexpr int kSmemBytes = kRawBytes + kTileBytes + kExchBytes + 512 * 2 + 256 * 2 + 16;
+constexpr int kTmemCols = 256;                   // 4 warps per lane quarter x 64 fp32 columns
 
 struct Params {
     const uint8_t *in;        // [C][T][2048]
@@ -124,12 +125,29 @@ __device__ __forceinline__ void mma_m16n8k8(float (&d)[4], uint32_t a0, uint32_t
                  : "r"(a0), "r"(a1), "r"(b));
 }
 
+// ---- tensor memory as a per-thread parking lot (32x32b shape: lane i of the warp <-> TMEM lane base + i) ----
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, float a0, float a1, float a2, float a3, float a4,
+                                         float a5, float a6, float a7) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 :: "r"(taddr), "f"(a0), "f"(a1), "f"(a2), "f"(a3), "f"(a4), "f"(a5), "f"(a6), "f"(a7) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float *v) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                 "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+                 "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]),
+                   "=f"(v[8]), "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15]),
+                   "=f"(v[16]), "=f"(v[17]), "=f"(v[18]), "=f"(v[19]), "=f"(v[20]), "=f"(v[21]), "=f"(v[22]), "=f"(v[23]),
+                   "=f"(v[24]), "=f"(v[25]), "=f"(v[26]), "=f"(v[27]), "=f"(v[28]), "=f"(v[29]), "=f"(v[30]), "=f"(v[31])
+                 : "r"(taddr) : "memory");
+}
+
 // ---- phase A ---------------------------------------------------------------------------------------
 // Warp w owns feeds n = 16 w .. 16 w + 15; lane = 4 g + tq is the mma fragment lane: time rows u' = g and
 // g + 8, cylinder tq.  raw: [piece p = 4 t + cyl][256 B], 8-byte units XOR-swizzled with (p & 15).
 template <int RHO>
 __device__ __forceinline__ void phase_a(const unsigned char *raw, float2 *tile, const uint2 *bfrag_cpe,
-                                        const int warp, const int lane) {
+                                        const int warp, const int lane, const uint32_t taddr) {
     constexpr bool ODD = (RHO & 1) != 0;
     const int g = lane >> 2, tq = lane & 3;
     const __half2 nbE = __floats2half2_rn(-32.0f / 512.0f, -32.0f / 512.0f);
@@ -185,24 +203,19 @@ __device__ __forceinline__ void phase_a(const unsigned char *raw, float2 *tile, 
             bw[i] = has_b ? __ldg(bfrag_cpe + (size_t)(n0 + i) * 16 + lane) : make_uint2(0u, 0u);
 #pragma unroll
         for (int i = 0; i < 8; i += 2) {
-            float z[2][4];
+            float z[2][4], zh[2][4];
 #pragma unroll
             for (int ii = 0; ii < 2; ++ii) {
-                float pacc[4] = {0.f, 0.f, 0.f, 0.f};
+                float pacc[4] = {0.f, 0.f, 0.f, 0.f}, qacc[4] = {0.f, 0.f, 0.f, 0.f};
                 mma_m16n8k8(pacc, aE[0][i + ii], aE[1][i + ii], bw[i + ii].x);
                 mma_m16n8k8(pacc, aE[0][i + ii], aE[1][i + ii], bw[i + ii].y);
-                if constexpr (ODD) {
-                    float qacc[4] = {0.f, 0.f, 0.f, 0.f};
-                    mma_m16n8k8(qacc, aO[0][i + ii], aO[1][i + ii], bw[i + ii].x);
-                    mma_m16n8k8(qacc, aO[0][i + ii], aO[1][i + ii], bw[i + ii].y);
-                    constexpr float s = 0.70710678118654752440f;
+                mma_m16n8k8(qacc, aO[0][i + ii], aO[1][i + ii], bw[i + ii].x);
+                mma_m16n8k8(qacc, aO[0][i + ii], aO[1][i + ii], bw[i + ii].y);
+                constexpr float s = ODD ? 0.70710678118654752440f : 1.0f;
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) z[ii][c] = fmaf(s, qacc[c], pacc[c]);
-                } else {
-                    mma_m16n8k8(pacc, aO[0][i + ii], aO[1][i + ii], bw[i + ii].x);
-                    mma_m16n8k8(pacc, aO[0][i + ii], aO[1][i + ii], bw[i + ii].y);
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) z[ii][c] = pacc[c];
+                for (int c = 0; c < 4; ++c) {
+                    z[ii][c] = fmaf(s, qacc[c], pacc[c]);    // residue RHO:      E + W_8^RHO O
+                    zh[ii][c] = fmaf(-s, qacc[c], pacc[c]);  // residue RHO + 4:  E - W_8^RHO O
                 }
             }
             if (stores) {
@@ -210,7 +223,34 @@ __device__ __forceinline__ void phase_a(const unsigned char *raw, float2 *tile, 
                 *reinterpret_cast<float4 *>(dst) = make_float4(z[0][0], z[0][1], z[1][0], z[1][1]);
                 *reinterpret_cast<float4 *>(dst + 16 * 2048) = make_float4(z[0][2], z[0][3], z[1][2], z[1][3]);
             }
+            // stash the RHO + 4 tile values in this thread's tensor-memory lane (32 columns per hh)
+            tmem_st8(taddr + 32 * hh + 4 * i, zh[0][0], zh[0][1], zh[1][0], zh[1][1], zh[0][2], zh[0][3], zh[1][2], zh[1][3]);
         }
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+
+// Phase A of residue RHO + 4: the tile values were computed with residue RHO (same integer butterflies,
+// same tensor-core products, opposite sign of the odd-tap half) and parked in tensor memory.
+__device__ __forceinline__ void phase_a_from_tmem(float2 *tile, const uint32_t taddr, const int warp, const int lane) {
+    const int g = lane >> 2, tq = lane & 3;
+    const int r0 = g * 2 + tq;
+    unsigned char *tile_t = reinterpret_cast<unsigned char *>(tile) + r0 * 2048 + warp * 128;
+    const int rx16 = (r0 & 7) << 4;
+    float v[64];
+    tmem_ld32(taddr, v);
+    tmem_ld32(taddr + 32, v + 32);
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    if (tq < 2) {
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+            for (int i = 0; i < 8; i += 2) {
+                const float *w = v + 32 * hh + 4 * i;
+                unsigned char *dst = tile_t + (rx16 ^ ((4 * hh + i / 2) << 4));
+                *reinterpret_cast<float4 *>(dst) = make_float4(w[0], w[1], w[2], w[3]);
+                *reinterpret_cast<float4 *>(dst + 16 * 2048) = make_float4(w[4], w[5], w[6], w[7]);
+            }
     }
 }
 
@@ -294,10 +334,6 @@ __device__ __forceinline__ void phase_c(const unsigned char *S, const int col, f
     }
 }
 
-template <int RHO>
-__device__ __forceinline__ void phase_a_rho(const unsigned char *raw, float2 *tile, const uint2 *bf, int warp, int lane) {
-    phase_a<RHO>(raw, tile, bf, warp, lane);
-}
 
 __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params prm) {
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -307,6 +343,7 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
     constexpr int kTileOfs = kRawBytes, kExchOfs = kRawBytes + kTileBytes;
     int16_t *s_sel = reinterpret_cast<int16_t *>(smem + kRawBytes + kTileBytes + kExchBytes);  // [32][16]
     int16_t *s_slot_of_m = s_sel + 512;                                          // [256]
+    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(s_slot_of_m + 256);          // TMEM base address
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ep = blockIdx.x & 1;
@@ -319,6 +356,17 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
         s_sel[tid] = prm.slot[(size_t)c * 512 + 2 * (16 * bitrev(i, 4) + (hl & 15)) + (hl >> 4)];
     }
     if (tid < 256) s_slot_of_m[tid] = prm.slot_of_m[(size_t)c * 256 + tid];
+    if (warp == 0) {   // one warp allocates 256 columns of tensor memory (1 CTA per SM: no contention)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                     :: "r"((uint32_t)__cvta_generic_to_shared(s_tmem)), "n"(kTmemCols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *s_tmem;
+    // a warp may touch only TMEM lanes 32 (warp % 4) .. +31; the 4 warps of a lane quarter take 64 columns each
+    const uint32_t taddr = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + 64u * (uint32_t)(warp >> 2);
 
     // phase B per-thread constants (rows warp and warp + 16 share the swizzle rx = warp & 7)
     const int h = lane >> 4, l = lane & 15;
@@ -370,16 +418,15 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
         const uint2 *bf = prm.bfrag + ((((size_t)c * 2 + pol) * 2 + ep) * 256) * 16;
 
 #pragma unroll 1
-        for (int rho = 0; rho < 8; ++rho) {
+        for (int it = 0; it < 8; ++it) {
+            // residues in the order 0, 4, 1, 5, 2, 6, 3, 7: RHO + 4 reuses the work of RHO (tensor-memory stash)
+            const int rho = (it >> 1) + 4 * (it & 1);
             switch (rho) {
-                case 0: phase_a_rho<0>(raw, tile, bf, warp, lane); break;
-                case 1: phase_a_rho<1>(raw, tile, bf, warp, lane); break;
-                case 2: phase_a_rho<2>(raw, tile, bf, warp, lane); break;
-                case 3: phase_a_rho<3>(raw, tile, bf, warp, lane); break;
-                case 4: phase_a_rho<4>(raw, tile, bf, warp, lane); break;
-                case 5: phase_a_rho<5>(raw, tile, bf, warp, lane); break;
-                case 6: phase_a_rho<6>(raw, tile, bf, warp, lane); break;
-                default: phase_a_rho<7>(raw, tile, bf, warp, lane); break;
+                case 0: phase_a<0>(raw, tile, bf, warp, lane, taddr); break;
+                case 1: phase_a<1>(raw, tile, bf, warp, lane, taddr); break;
+                case 2: phase_a<2>(raw, tile, bf, warp, lane, taddr); break;
+                case 3: phase_a<3>(raw, tile, bf, warp, lane, taddr); break;
+                default: phase_a_from_tmem(tile, taddr, warp, lane); break;
             }
             __syncthreads();
             {
@@ -402,6 +449,9 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
             __syncthreads();
         }
     }
+    // tensor memory is released by the warp that allocated it, after every warp's last tcgen05.ld
+    if (warp == 0)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "n"(kTmemCols));
 
     // ---- epilogue: thread <-> (e', slot) -> beam m ----
     const int e = 2 * ep + e1;
