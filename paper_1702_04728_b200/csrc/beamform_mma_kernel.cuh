@@ -264,9 +264,9 @@ __device__ __forceinline__ void phase_a_from_tmem(float2 *tile, const uint32_t t
 //   exch read     ex + (er ^ (i << 4)),        er = 128 l | (((l&7) ^ x) << 4)
 // with rx = r & 7 (the row's swizzle; identical for the warp's two rows r and r + 16), x = rx (even half,
 // exchanging through the row) or 0 (odd half, private buffer).
-// s_sel[(16 h + l) * 16 + i] = slot of bin 2 (16 bitrev(i) + l) + h, or -1; slot -> byte (slot ^ (rx << 1)) * 8.
+// s_sel[(16 h + l) * 16 + i] = 8 * slot of bin 2 (16 bitrev(i) + l) + h, or 0x8000 (not selected).
 __device__ __forceinline__ void phase_b_row(unsigned char *S, const int rowofs, const int exofs, const int h,
-                                            const int rd, const int wr, const int er, const int rx2,
+                                            const int rd, const int wr, const int er,
                                             const uint4 sel0, const uint4 sel1, const float2 (&twc)[16]) {
     float2 a[16];
     const int ra = rowofs + rd;
@@ -297,11 +297,15 @@ __device__ __forceinline__ void phase_b_row(unsigned char *S, const int rowofs, 
     }
     fft_dif<16>(b);
     __syncwarp();  // all exchange reads done before slots are written into the row
+    // sel: per output i a 16-bit byte offset of its slot inside the row (slot * 8, row swizzle already applied
+    // by the caller) or 0x8000 if the bin is not selected
     const uint32_t sw[8] = {sel0.x, sel0.y, sel0.z, sel0.w, sel1.x, sel1.y, sel1.z, sel1.w};
+    unsigned char *rowp = S + rowofs;
 #pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const int s = (int)(int16_t)((i & 1) ? (sw[i >> 1] >> 16) : (sw[i >> 1] & 0xFFFFu));
-        if (s >= 0) *reinterpret_cast<float2 *>(S + (rowofs + ((s ^ rx2) << 3))) = b[i];
+    for (int i = 0; i < 16; i += 2) {
+        const uint32_t w = sw[i >> 1];
+        if (!(w & 0x8000u)) *reinterpret_cast<float2 *>(rowp + (w & 0xFFFFu)) = b[i];
+        if ((int)w >= 0) *reinterpret_cast<float2 *>(rowp + (w >> 16)) = b[i + 1];
     }
 }
 
@@ -353,7 +357,8 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
 
     {   // s_sel[(16 h + l) * 16 + i] = slot of bin 2 (16 bitrev(i) + l) + h
         const int i = tid & 15, hl = tid >> 4;
-        s_sel[tid] = prm.slot[(size_t)c * 512 + 2 * (16 * bitrev(i, 4) + (hl & 15)) + (hl >> 4)];
+        const int sl0 = prm.slot[(size_t)c * 512 + 2 * (16 * bitrev(i, 4) + (hl & 15)) + (hl >> 4)];
+        s_sel[tid] = (int16_t)(sl0 < 0 ? 0x8000 : sl0 * 8);
     }
     if (tid < 256) s_slot_of_m[tid] = prm.slot_of_m[(size_t)c * 256 + tid];
     if (warp == 0) {   // one warp allocates 256 columns of tensor memory (1 CTA per SM: no contention)
@@ -430,10 +435,14 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
             }
             __syncthreads();
             {
-                const uint4 sel0 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16);
-                const uint4 sel1 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16 + 8);
-                phase_b_row(S, row0, h ? exw : row0, h, rd, wr, er, rx << 1, sel0, sel1, twc);
-                phase_b_row(S, row1, h ? exw : row1, h, rd, wr, er, rx << 1, sel0, sel1, twc);
+                // slot byte offsets of this lane's 16 outputs, with the rows' chunk swizzle (rx << 4) applied
+                const uint32_t xr = (uint32_t)(rx << 4) * 0x00010001u;
+                uint4 sel0 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16);
+                uint4 sel1 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16 + 8);
+                sel0 = make_uint4(sel0.x ^ xr, sel0.y ^ xr, sel0.z ^ xr, sel0.w ^ xr);
+                sel1 = make_uint4(sel1.x ^ xr, sel1.y ^ xr, sel1.z ^ xr, sel1.w ^ xr);
+                phase_b_row(S, row0, h ? exw : row0, h, rd, wr, er, sel0, sel1, twc);
+                phase_b_row(S, row1, h ? exw : row1, h, rd, wr, er, sel0, sel1, twc);
             }
             __syncthreads();
             switch (rho) {
