@@ -14,6 +14,7 @@
 
 #include "beamform_kernel.cuh"
 #include "beamform_mma_kernel.cuh"
+#include "beamform_ws_kernel.cuh"
 
 namespace {
 
@@ -43,6 +44,7 @@ struct chime_bf_plan {
     float2 *d_tw_u = nullptr;
     uint2 *d_bfrag = nullptr;  // tensor-core B fragments of the folded weights (zero_pad 512, upchan 128 path)
     bool use_mma = false;
+    bool use_ws = false;       // warp-specialised variant of the tensor-core path
     // staging for execute_host
     uint8_t *d_stage_in = nullptr;
     uint8_t *d_stage_out = nullptr;
@@ -173,6 +175,8 @@ bool build_tables(chime_bf_plan *pl, const chime_bf_params &p, double fref, doub
         CUDA_TRY(cudaMemcpyToSymbol(chime2::c_tw128, tw128.data(), sizeof(float2) * 128));
         CUDA_TRY(cudaFuncSetAttribute(chime2::beamform_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       chime2::kSmemBytes));
+        CUDA_TRY(cudaFuncSetAttribute(chime3::beamform_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      chime3::kSmemBytesWs));
         if (!upload(&pl->d_bfrag, bfrag)) return false;
     }
     return upload(&pl->d_wp, wp) && upload(&pl->d_slot, slot) && upload(&pl->d_slot_of_m, slot_of_m) &&
@@ -231,7 +235,10 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         mp.norm = pl->norm;
         mp.qscale = pl->norm * pl->scale;
         mp.qoffset = pl->offset;
-        chime2::beamform_mma_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
+        if (pl->use_ws)
+            chime3::beamform_ws_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
+        else
+            chime2::beamform_mma_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
         const cudaError_t e2 = cudaGetLastError();
         if (e2 != cudaSuccess) {
             set_err("kernel launch failed: %s", cudaGetErrorString(e2));
@@ -299,6 +306,7 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     pl->scale = p.scale > 0.f ? p.scale : 1.0f / 64.0f;
     pl->offset = p.scale > 0.f ? p.offset : 128.0f;
     pl->norm = (float)(1.0 / (256.0 * 4.0 * (double)p.upchan_len));
+    pl->use_ws = !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v2"));
     pl->use_mma = (p.zero_pad == 512 && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
     cudaGetDevice(&pl->device);
     const double fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
