@@ -265,6 +265,15 @@ __device__ __forceinline__ void phase_a_from_tmem(float2 *tile, const uint32_t t
 // with rx = r & 7 (the row's swizzle; identical for the warp's two rows r and r + 16), x = rx (even half,
 // exchanging through the row) or 0 (odd half, private buffer).
 // s_sel[(16 h + l) * 16 + i] = 8 * slot of bin 2 (16 bitrev(i) + l) + h, or 0x8000 (not selected).
+// a[k] *= W_32^k (the compile-time part of the odd-bin pre-twiddle W_512^{l + 16 k})
+__device__ __forceinline__ void w32_pretwiddle(float2 (&a)[16]) {
+    a[1] = chime::twiddle64<2>(a[1]);   a[2] = chime::twiddle64<4>(a[2]);   a[3] = chime::twiddle64<6>(a[3]);
+    a[4] = chime::twiddle64<8>(a[4]);   a[5] = chime::twiddle64<10>(a[5]);  a[6] = chime::twiddle64<12>(a[6]);
+    a[7] = chime::twiddle64<14>(a[7]);  a[8] = chime::twiddle64<16>(a[8]);  a[9] = chime::twiddle64<18>(a[9]);
+    a[10] = chime::twiddle64<20>(a[10]); a[11] = chime::twiddle64<22>(a[11]); a[12] = chime::twiddle64<24>(a[12]);
+    a[13] = chime::twiddle64<26>(a[13]); a[14] = chime::twiddle64<28>(a[14]); a[15] = chime::twiddle64<30>(a[15]);
+}
+
 __device__ __forceinline__ void phase_b_row(unsigned char *S, const int rowofs, const int exofs, const int h,
                                             const int rd, const int wr, const int er,
                                             const uint4 sel0, const uint4 sel1, const float2 (&twc)[16]) {

@@ -24,7 +24,7 @@ using namespace chime2;
 
 constexpr int kConsumerWarps = 8, kProducerWarps = 8;
 constexpr int kCThreads = 32 * kConsumerWarps, kPThreads = 32 * kProducerWarps;
-constexpr int kExchBytesWs = kConsumerWarps * 2048;   // 16 KiB
+constexpr int kExchBytesWs = kConsumerWarps * 2 * 2048;   // 32 KiB: two rows in flight per consumer warp
 constexpr int kSmemBytesWs = kRawBytes + kTileBytes + kExchBytesWs + 512 * 2 + 256 * 2 + 16;
 
 // named barriers (0 is __syncthreads)
@@ -129,6 +129,85 @@ __device__ __forceinline__ void tile_from_tmem(unsigned char *S, const int tile_
     }
 }
 
+// ---- consumer phase B on TWO tile rows at once (same lane constants; independent instruction streams
+// give the two consumer warps of an SM sub-partition the instruction-level parallelism of four) -----------
+__device__ __forceinline__ void phase_b_2rows(unsigned char *S, const int rowA, const int rowB, const int exA,
+                                              const int exB, const int h, const int rd, const int wr, const int er,
+                                              const uint4 sel0, const uint4 sel1, const float2 (&twc)[16]) {
+    float2 a0[16], a1[16];
+    const int ra0 = rowA + rd, ra1 = rowB + rd;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        a0[k] = *reinterpret_cast<const float2 *>(S + (ra0 + 128 * k));
+        a1[k] = *reinterpret_cast<const float2 *>(S + (ra1 + 128 * k));
+    }
+    if (h) {
+        w32_pretwiddle(a0);
+        w32_pretwiddle(a1);
+    }
+    fft_dif<16>(a0);
+    fft_dif<16>(a1);
+    __syncwarp();  // every lane has read both rows before the even half overwrites them
+    const int wa0 = exA + wr, wa1 = exB + wr, ea0 = exA + er, ea1 = exB + er;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const int j2 = bitrev(i, 4);
+        *reinterpret_cast<float2 *>(S + ((wa0 ^ ((j2 & 7) << 4)) + 128 * j2)) = cmul(a0[i], twc[j2]);
+        *reinterpret_cast<float2 *>(S + ((wa1 ^ ((j2 & 7) << 4)) + 128 * j2)) = cmul(a1[i], twc[j2]);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float4 v = *reinterpret_cast<const float4 *>(S + (ea0 ^ (i << 4)));
+        const float4 w = *reinterpret_cast<const float4 *>(S + (ea1 ^ (i << 4)));
+        a0[2 * i] = make_float2(v.x, v.y);
+        a0[2 * i + 1] = make_float2(v.z, v.w);
+        a1[2 * i] = make_float2(w.x, w.y);
+        a1[2 * i + 1] = make_float2(w.z, w.w);
+    }
+    fft_dif<16>(a0);
+    fft_dif<16>(a1);
+    __syncwarp();  // all exchange reads done before slots are written into the rows
+    const uint32_t sw[8] = {sel0.x, sel0.y, sel0.z, sel0.w, sel1.x, sel1.y, sel1.z, sel1.w};
+    unsigned char *rp0 = S + rowA, *rp1 = S + rowB;
+#pragma unroll
+    for (int i = 0; i < 16; i += 2) {
+        const uint32_t w = sw[i >> 1];
+        if (!(w & 0x8000u)) {
+            *reinterpret_cast<float2 *>(rp0 + (w & 0xFFFFu)) = a0[i];
+            *reinterpret_cast<float2 *>(rp1 + (w & 0xFFFFu)) = a1[i];
+        }
+        if ((int)w >= 0) {
+            *reinterpret_cast<float2 *>(rp0 + (w >> 16)) = a0[i + 1];
+            *reinterpret_cast<float2 *>(rp1 + (w >> 16)) = a1[i + 1];
+        }
+    }
+}
+
+// ---- consumer phase C on the thread's two columns (beams e' = 0, 1 of one slot) at once ------------------
+template <int RHO>
+__device__ __forceinline__ void phase_c2(const unsigned char *S, const int col0, const int col1, float (&acc0)[16],
+                                         float (&acc1)[16]) {
+    float2 a0[16], a1[16];
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+        a0[u] = *reinterpret_cast<const float2 *>(S + ((col0 ^ ((2 * (u & 3)) << 4)) + 4096 * u));
+        a1[u] = *reinterpret_cast<const float2 *>(S + ((col1 ^ ((2 * (u & 3)) << 4)) + 4096 * u));
+    }
+    if constexpr (RHO != 0) {
+        time_pretwiddle<RHO, 1>(a0);
+        time_pretwiddle<RHO, 1>(a1);
+    }
+    fft_dif<16>(a0);
+    fft_dif<16>(a1);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const int g = (bitrev(i, 4) + 8) & 15;
+        acc0[g] = fmaf(a0[i].x, a0[i].x, fmaf(a0[i].y, a0[i].y, acc0[g]));
+        acc1[g] = fmaf(a1[i].x, a1[i].x, fmaf(a1[i].y, a1[i].y, acc1[g]));
+    }
+}
+
 __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params prm) {
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *const S = smem;
@@ -166,6 +245,7 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
 
     if (warp >= kConsumerWarps) {
         // ======================================= PRODUCERS =======================================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
         const int ptid = tid - kCThreads;
 #pragma unroll 1
         for (int blk = 0; blk < 6; ++blk) {
@@ -213,13 +293,14 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
         }
     } else {
         // ======================================= CONSUMERS =======================================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 168;");
         const int h = lane >> 4, l = lane & 15;
         const int rx = rw & 7, xx = h ? 0 : rx;   // rows rw, rw + 8, rw + 16, rw + 24 share the swizzle
         const int rd = (((l >> 1) ^ rx) << 4) | ((l & 1) << 3);
         const int wr = (((l >> 1) ^ xx) << 4) | ((l & 1) << 3);
         const int er = (128 * l) | (((l & 7) ^ xx) << 4);
         const int row0 = kTileOfs + rw * 2048;
-        const int exw = kExchOfs + rw * 2048;
+        const int exw = kExchOfs + rw * 4096;
         float2 twc[16];
 #pragma unroll
         for (int j2 = 0; j2 < 16; ++j2) twc[j2] = __ldg(prm.tw_np + ((l * (2 * j2 + h)) & 511));
@@ -251,21 +332,21 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
                     sel0 = make_uint4(sel0.x ^ xr, sel0.y ^ xr, sel0.z ^ xr, sel0.w ^ xr);
                     sel1 = make_uint4(sel1.x ^ xr, sel1.y ^ xr, sel1.z ^ xr, sel1.w ^ xr);
 #pragma unroll 1
-                    for (int rr = 0; rr < 4; ++rr) {
-                        const int rowofs = row0 + rr * 8 * 2048;
-                        phase_b_row(S, rowofs, h ? exw : rowofs, h, rd, wr, er, sel0, sel1, twc);
+                    for (int rr = 0; rr < 4; rr += 2) {
+                        const int rowA = row0 + rr * 8 * 2048, rowB = rowA + 8 * 2048;
+                        phase_b_2rows(S, rowA, rowB, h ? exw : rowA, h ? exw + 2048 : rowB, h, rd, wr, er, sel0, sel1, twc);
                     }
                 }
                 bar_sync(BAR_CONS, kCThreads);
                 switch (pr + 4 * half) {
-                    case 0: phase_c<0>(S, col0, acc0); phase_c<0>(S, col1, acc1); break;
-                    case 1: phase_c<1>(S, col0, acc0); phase_c<1>(S, col1, acc1); break;
-                    case 2: phase_c<2>(S, col0, acc0); phase_c<2>(S, col1, acc1); break;
-                    case 3: phase_c<3>(S, col0, acc0); phase_c<3>(S, col1, acc1); break;
-                    case 4: phase_c<4>(S, col0, acc0); phase_c<4>(S, col1, acc1); break;
-                    case 5: phase_c<5>(S, col0, acc0); phase_c<5>(S, col1, acc1); break;
-                    case 6: phase_c<6>(S, col0, acc0); phase_c<6>(S, col1, acc1); break;
-                    default: phase_c<7>(S, col0, acc0); phase_c<7>(S, col1, acc1); break;
+                    case 0: phase_c2<0>(S, col0, col1, acc0, acc1); break;
+                    case 1: phase_c2<1>(S, col0, col1, acc0, acc1); break;
+                    case 2: phase_c2<2>(S, col0, col1, acc0, acc1); break;
+                    case 3: phase_c2<3>(S, col0, col1, acc0, acc1); break;
+                    case 4: phase_c2<4>(S, col0, col1, acc0, acc1); break;
+                    case 5: phase_c2<5>(S, col0, col1, acc0, acc1); break;
+                    case 6: phase_c2<6>(S, col0, col1, acc0, acc1); break;
+                    default: phase_c2<7>(S, col0, col1, acc0, acc1); break;
                 }
                 bar_sync(BAR_CONS, kCThreads);
             }

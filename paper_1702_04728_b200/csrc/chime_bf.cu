@@ -45,8 +45,8 @@ struct chime_bf_plan {
     float2 *d_tw_u = nullptr;
     uint2 *d_bfrag = nullptr;  // tensor-core B fragments of the folded weights (zero_pad 512, upchan 128 path)
     bool use_mma = false;
-    bool use_ws = false;
-    bool use_il = false;       // interleaved-schedule variant (default)       // warp-specialised variant of the tensor-core path
+    bool use_ws = false;       // warp-specialised variant of the tensor-core path (default)
+    bool use_il = false;       // interleaved-schedule variant (CHIME_BF_KERNEL=v4)
     // staging for execute_host
     uint8_t *d_stage_in = nullptr;
     uint8_t *d_stage_out = nullptr;
@@ -313,9 +313,9 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     pl->offset = p.scale > 0.f ? p.offset : 128.0f;
     pl->norm = (float)(1.0 / (256.0 * 4.0 * (double)p.upchan_len));
     {
-        const char *kv = getenv("CHIME_BF_KERNEL");   // A/B switch: v1 generic, v2 mma, v3 warp-specialised, v4 interleaved
-        pl->use_il = !kv || !strcmp(kv, "v4");
-        pl->use_ws = kv && !strcmp(kv, "v3");
+        const char *kv = getenv("CHIME_BF_KERNEL");   // A/B switch: v1 generic, v2 mma, v3 warp-specialised (default), v4 interleaved
+        pl->use_ws = !kv || !strcmp(kv, "v3");
+        pl->use_il = kv && !strcmp(kv, "v4");
     }
     pl->use_mma = (p.zero_pad == 512 && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
     cudaGetDevice(&pl->device);

@@ -149,3 +149,23 @@ def test_cfg1_full_size_sampled(bf, orc):
 
     worst, frac = compare_cells(orc, plan, d_in, host_bytes, freqs, gains, cells, 512, 128)
     print(f"cfg1: worst rel err {worst:.2e}, u8 diff frac {frac:.2e}")
+
+
+@pytest.mark.parametrize("kernel", ["v1", "v2", "v3", "v4"])
+def test_all_kernel_generations_agree_with_oracle(bf, orc, kernel, monkeypatch):
+    """The library keeps four generations of the zero_pad 512 / upchan 128 kernel behind CHIME_BF_KERNEL
+    (v1 generic fp32, v2 tensor-core E-W, v3 warp-specialised [default], v4 interleaved): each must meet the
+    same tolerances on cfg0 plus a random-gain channel with a ragged frame count."""
+    monkeypatch.setenv("CHIME_BF_KERNEL", kernel)
+    seed = synth.config_seed(1)
+    C, T = 2, 3 * 384
+    freqs = np.array([800.0, 437.890625])
+    gains = synth.gains(seed, C, flagged_frac=0.02)
+    b = synth.noise_bytes(seed, C, T)
+    plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, n_time=T)
+    hb = b.numpy()
+    cells = [(0, 0), (0, 2), (1, 1)]
+    worst, frac = compare_cells(orc, plan, b.cuda(), lambda c, R: hb[c, 384 * R:384 * (R + 1)], freqs, gains,
+                                cells, 512, 128)
+    print(f"{kernel}: worst rel err {worst:.2e}, u8 diff frac {frac:.2e}")
+    plan.destroy()
