@@ -15,7 +15,6 @@
 #include "beamform_kernel.cuh"
 #include "beamform_mma_kernel.cuh"
 #include "beamform_ws_kernel.cuh"
-#include "beamform_il_kernel.cuh"
 
 namespace {
 
@@ -46,7 +45,6 @@ struct chime_bf_plan {
     uint2 *d_bfrag = nullptr;  // tensor-core B fragments of the folded weights (zero_pad 512, upchan 128 path)
     bool use_mma = false;
     bool use_ws = false;       // warp-specialised variant of the tensor-core path (default)
-    bool use_il = false;       // interleaved-schedule variant (CHIME_BF_KERNEL=v4)
     // staging for execute_host
     uint8_t *d_stage_in = nullptr;
     uint8_t *d_stage_out = nullptr;
@@ -177,8 +175,6 @@ bool build_tables(chime_bf_plan *pl, const chime_bf_params &p, double fref, doub
         CUDA_TRY(cudaMemcpyToSymbol(chime2::c_tw128, tw128.data(), sizeof(float2) * 128));
         CUDA_TRY(cudaFuncSetAttribute(chime2::beamform_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       chime2::kSmemBytes));
-        CUDA_TRY(cudaFuncSetAttribute(chime4::beamform_il_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      chime2::kSmemBytes));
         CUDA_TRY(cudaFuncSetAttribute(chime3::beamform_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       chime3::kSmemBytesWs));
         if (!upload(&pl->d_bfrag, bfrag)) return false;
@@ -239,9 +235,7 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         mp.norm = pl->norm;
         mp.qscale = pl->norm * pl->scale;
         mp.qoffset = pl->offset;
-        if (pl->use_il)
-            chime4::beamform_il_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
-        else if (pl->use_ws)
+        if (pl->use_ws)
             chime3::beamform_ws_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
         else
             chime2::beamform_mma_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
@@ -313,9 +307,8 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     pl->offset = p.scale > 0.f ? p.offset : 128.0f;
     pl->norm = (float)(1.0 / (256.0 * 4.0 * (double)p.upchan_len));
     {
-        const char *kv = getenv("CHIME_BF_KERNEL");   // A/B switch: v1 generic, v2 mma, v3 warp-specialised (default), v4 interleaved
+        const char *kv = getenv("CHIME_BF_KERNEL");   // A/B switch: v1 generic, v2 block-synchronous mma, v3 warp-specialised (default)
         pl->use_ws = !kv || !strcmp(kv, "v3");
-        pl->use_il = kv && !strcmp(kv, "v4");
     }
     pl->use_mma = (p.zero_pad == 512 && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
     cudaGetDevice(&pl->device);
