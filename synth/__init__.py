@@ -130,16 +130,17 @@ def gains(seed, n_chan, flagged_frac=0.02, amp_lo=0.8, amp_hi=1.2):
     return g.to(torch.float32).reshape(n_chan, N_INPUT, 2).numpy()
 
 
-def saturate_bursts(b, seed, frac=0.05, burst=64):
+def saturate_bursts(b, seed, frac=0.05, burst=64, inplace=False):
     """cfg4 RFI: a fraction `frac` of time samples, in bursts of `burst` consecutive samples, have
-    every input's re and im set to +-7 with random signs.  b: [C][T][2048] uint8 (modified copy).
+    every input's re and im set to +-7 with random signs.  b: [C][T][2048] uint8 (a modified copy is
+    returned unless inplace=True: the 51 GB buffer of cfg4 is not cloned).
     Returns (bytes, burst_mask [C][T] bool)."""
     C, T, _ = b.shape
     dev = b.device
     nb = (T + burst - 1) // burst
     u = uniform01(seed, C * nb, 20, dev).reshape(C, nb)
     mask = (u < frac).repeat_interleave(burst, dim=1)[:, :T]
-    out = b.clone()
+    out = b if inplace else b.clone()
     for c in range(C):
         ts = torch.nonzero(mask[c]).flatten()
         if ts.numel() == 0:
@@ -150,6 +151,75 @@ def saturate_bursts(b, seed, frac=0.05, burst=64):
         im = torch.where((h & 2) == 0, 15, 1)
         out[c, ts] = ((re << 4) | im).to(torch.uint8)
     return out, mask
+
+
+K_DM_MS = 4.148808          # dispersion constant: delay = K_DM_MS ms * DM * (f/GHz)^-2
+SAMPLE_S = 2.56e-6          # PAPER.md:37 (Table 1)
+
+
+def pulse_centres(freqs_mhz, n_time, dm=500.0, t0_samples=1000.0, f_top_mhz=800.0):
+    """cfg2: arrival time (in samples, float64) of a dispersed pulse in each coarse channel,
+    t0 + K_DM*DM*(f^-2 - f_top^-2), wrapped modulo the n_time window so that every channel contains
+    the pulse (the 9.7 s sweep of DM 500 over 400-800 MHz is longer than the 1 s buffer)."""
+    f = np.asarray(freqs_mhz, dtype=np.float64) / 1e3
+    delay_s = K_DM_MS * 1e-3 * dm * (f ** -2 - (f_top_mhz / 1e3) ** -2)
+    return np.mod(t0_samples + delay_s / SAMPLE_S, float(n_time))
+
+
+def pulse_amplitude_var(snr=20.0, width_samples=390.625, sigma_in2=12.556, n_inputs_per_pol=1024):
+    """Peak per-input variance p0 of the pulse voltage such that the matched-filter S/N of the
+    16-fine-channel-summed intensity of the on-source beam is `snr` in one coarse channel:
+      signal = 2 pol * N*N_c * sum_t p(t) = 2*1024 * 1.0645 p0 w      (Gaussian envelope, FWHM w)
+      noise  = sigma_in^2 * sqrt(2 pol * w)                          (|.|^2 of Gaussian noise, w samples)
+    sigma_in2 = variance of one complex noise sample (re + im) of round(N(0, 2.5)) clipped."""
+    w = width_samples
+    return snr * sigma_in2 * math.sqrt(2.0 * w) / (2.0 * n_inputs_per_pol * 1.0645 * w)
+
+
+def add_pulse(b, seed, freqs_mhz, gains=None, sin_theta=0.0, sin_phi=0.0, dm=500.0, snr=20.0,
+              width_s=1e-3, sigma=2.5, t0_samples=1000.0, feed_spacing_m=0.3048, cyl_spacing_m=22.0,
+              half_window=640):
+    """cfg2: adds a dispersed, noise-like (FRB-like) pulse from direction (sin_theta, sin_phi) to the
+    packed baseband b [C][T][2048] IN PLACE and returns the per-channel pulse centres (samples).
+
+    Inside a window of +-half_window samples around each channel's arrival time the samples are redrawn
+    as  pack(round(clip( N(0, sigma) noise + h_i * a(t) s(t) * geometric phase ))), i.e. the pulse is added
+    BEFORE the 4-bit quantisation.  s(t) is one complex Gaussian series common to all inputs, a(t) a
+    Gaussian envelope of FWHM width_s, h_i = 1/g_i the instrumental response that the plan's calibration
+    gain g_i undoes (flagged inputs, g = 0, carry noise only).  The intra-channel dispersion chirp is
+    omitted (flagged simplification).  Windows that would cross the buffer ends are clipped."""
+    C, T, _ = b.shape
+    dev = b.device
+    w = width_s / SAMPLE_S
+    centres = pulse_centres(freqs_mhz, T, dm, t0_samples)
+    p0 = pulse_amplitude_var(snr, w)
+    n = torch.arange(256, dtype=torch.float64, device=dev).view(1, 1, 1, 256)
+    cyl = torch.arange(4, dtype=torch.float64, device=dev).view(1, 1, 4, 1)
+    for c in range(C):
+        lo = max(0, int(centres[c]) - half_window)
+        hi = min(T, int(centres[c]) + half_window)
+        L = hi - lo
+        shape = (L, 2, 4, 256)
+        nr = gaussian(seed + 7919 * (c + 1), shape, 0, dev) * sigma
+        ni = gaussian(seed + 7919 * (c + 1), shape, 1, dev) * sigma
+        t = torch.arange(lo, hi, dtype=torch.float64, device=dev)
+        env = torch.sqrt(p0 / 2.0 * torch.exp(-4.0 * math.log(2.0) * ((t - centres[c]) / w) ** 2))
+        sr = gaussian(seed + 7919 * (c + 1), (L,), 2, dev) * env
+        si = gaussian(seed + 7919 * (c + 1), (L,), 3, dev) * env
+        ph = 2.0 * math.pi * (float(freqs_mhz[c]) * 1e6 / C0) * (n * feed_spacing_m * sin_theta
+                                                                 + cyl * cyl_spacing_m * sin_phi)
+        hr, hi_ = torch.cos(ph), torch.sin(ph)                      # geometric phase [1][1][4][256]
+        if gains is not None:                                       # h = 1/g = conj(g)/|g|^2
+            g = torch.as_tensor(gains[c], dtype=torch.float64, device=dev).reshape(1, 2, 4, 256, 2)
+            g2 = g[..., 0] ** 2 + g[..., 1] ** 2
+            inv = torch.where(g2 > 0, 1.0 / torch.where(g2 > 0, g2, torch.ones_like(g2)), torch.zeros_like(g2))
+            ir, ii = g[..., 0] * inv, -g[..., 1] * inv
+            hr, hi_ = hr * ir - hi_ * ii, hr * ii + hi_ * ir
+        sr4, si4 = sr.view(L, 1, 1, 1), si.view(L, 1, 1, 1)
+        vr = nr + (hr * sr4 - hi_ * si4)
+        vi = ni + (hr * si4 + hi_ * sr4)
+        b[c, lo:hi] = pack_voltage(vr, vi).reshape(L, N_INPUT)
+    return centres
 
 
 def chime_freqs_mhz(n_coarse, step=1, k0=0):
