@@ -7,6 +7,7 @@ coarse channels that rate sustains in real time, 1 channel = 0.8 GB/s).
 
   python bench.py [--gpus N] [--steps K] [--warmup W]          CUDA arm
   python bench.py --impl reference ...                         oracle arm (CPU, bounded sample)
+  python bench.py --workload cfg3 [--chunks 80]                full-band streaming (configs[3]), 1 GPU
 """
 import argparse
 import json
@@ -292,6 +293,67 @@ def run_cuda(args):
     return 0
 
 
+def run_cfg3(args):
+    """--workload cfg3: BASELINE.json configs[3], full-band streaming.  1024 channels x 49152-sample chunks as
+    8 channel groups of 128 (12.9 GB each) through two device-resident buffers on two CUDA streams, looped
+    for --chunks full-band chunks (80 = 10.07 s of telescope time, 8.25 TB).  Host/PCIe ingest is not part
+    of it (819 GB/s cannot come from a host); the buffers hold seeded noise and are re-used."""
+    import torch
+
+    import paper_1702_04728_b200 as bf
+    import synth
+    from paper_1702_04728_b200.streaming import FullBandStreamer
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    bf.load_library()
+    cfg = synth.CONFIGS[3]
+    C, T, G = cfg["n_coarse"], cfg["n_time"], cfg["group"]
+    seed = synth.config_seed(3)
+    st = FullBandStreamer(C, G, T, freq_mhz=synth.config_freqs(3))
+    for i, buf in enumerate(st.in_bufs):
+        buf.copy_(synth.noise_bytes(seed, G, T, device="cuda", chan0=i * G))
+    outs = [torch.empty(st.group_out_shape, dtype=torch.uint8, device="cuda") for _ in range(st.n_groups)]
+    sampler = ClockSampler(0)
+    sampler.start()
+    st.run_chunk(None, out_u8=outs)                       # warm-up: one full-band chunk (8 launches)
+    st.synchronize()
+    torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True)
+    ends = [torch.cuda.Event(enable_timing=True) for _ in st.streams]
+    e0.record(st.streams[0])
+    st.streams[1].wait_event(e0)
+    st.launches = 0
+    for _ in range(args.chunks):
+        st.run_chunk(None, out_u8=outs)
+    for e, s in zip(ends, st.streams):
+        e.record(s)
+    st.synchronize()
+    torch.cuda.synchronize()
+    ms = max(e0.elapsed_time(e) for e in ends)
+    clocks = sampler.stop()
+    total_bytes = float(args.chunks) * C * T * BYTES_PER_CHAN_SAMPLE
+    gbs = total_bytes / (ms * 1e-3) / 1e9
+    tel_s = args.chunks * T / REALTIME_SAMPLES_PER_S
+    line = {
+        "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": 1, "steps": args.chunks, "warmup": 1,
+        "ms_per_step": ms / args.chunks, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "channels_realtime": gbs / GBS_PER_CHANNEL,
+        "realtime_fraction_full_band": gbs / (1024 * GBS_PER_CHANNEL),
+        "config": {"workload": "configs[3] full band streaming: 1024 coarse channels x 49152-sample chunks, "
+                               "8 channel groups of 128 on two streams / two device buffers (ping-pong), "
+                               f"{args.chunks} chunks = {tel_s:.2f} s of telescope time, {total_bytes / 1e12:.2f} TB",
+                   "telescope_seconds": tel_s, "wall_seconds": ms * 1e-3,
+                   "paper_rate": "6.4 Tbps = 800 GB/s as printed (PAPER.md:43); exact product 819.2 GB/s",
+                   "l2": "each group (12.9 GB) is far larger than L2"},
+        "gpu_launches": st.launches, "clocks": clocks,
+    }
+    print(json.dumps(line))
+    st.destroy()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -299,8 +361,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="cfg1", choices=["cfg1", "cfg3"],
+                    help="cfg1 (default, the contract's step) or cfg3 (full-band streaming, 1 GPU)")
+    ap.add_argument("--chunks", type=int, default=80, help="cfg3: full-band chunks to stream")
     args = ap.parse_args()
-    return run_reference(args) if args.impl == "reference" else run_cuda(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cfg3(args) if args.workload == "cfg3" else run_cuda(args)
 
 
 if __name__ == "__main__":
