@@ -100,6 +100,25 @@ int chime_bf_execute_f32(chime_bf_plan *plan, void *cuda_stream, const uint8_t *
 int chime_bf_execute_host(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8_host,
                           uint8_t *out_u8_host);
 
+/*
+ * Re-plannable tables (sec. 3.1: "The extent of the N-S horizon coverage is tunable, and we
+ * have the flexibility to form denser or sparser beam tilings.  ... the E-W formed beams can be configured
+ * as static or tracking"; gains: BASELINE.json).  Each call recomputes the affected host tables in double
+ * precision exactly as plan creation does and copies them into the plan's existing device allocations,
+ * ordered on `cuda_stream`: executes enqueued on that stream after the call see the new tables, executes
+ * enqueued before it the old ones.  The caller must not have executes of this plan in flight on OTHER
+ * streams.  No allocation, no plan rebuild.  Return CHIME_BF_OK or a negative code.
+ *   update_gains       gains: HOST [C][2048][2] float, copied; NULL = unit gains
+ *   update_ew_angles   ew_angles_deg: HOST [4] double (tracking E-W beams: call once per pointing update)
+ *   update_pointings   ns_sin_theta: HOST [256] double explicit pointings sin(theta_m) in [-1, 1], or NULL
+ *                      to use the native 256-point grid at f_ref_mhz (<= 0 keeps the current f_ref).
+ *                      Rebuilds the clamped index table J (eq. (1),(2)) and its slot maps.
+ */
+int chime_bf_update_gains(chime_bf_plan *plan, void *cuda_stream, const float *gains);
+int chime_bf_update_ew_angles(chime_bf_plan *plan, void *cuda_stream, const double *ew_angles_deg);
+int chime_bf_update_pointings(chime_bf_plan *plan, void *cuda_stream, double f_ref_mhz,
+                              const double *ns_sin_theta);
+
 /* Copy of the clamped N-S bin index table J (eq. (1),(2)): HOST out, [C][256] int32. */
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out);
 

@@ -18,7 +18,7 @@ EXPORTS = [
     "chime_bf_plan_create", "chime_bf_plan_create_ex", "chime_bf_execute", "chime_bf_execute_f32",
     "chime_bf_execute_host", "chime_bf_get_ns_index", "chime_bf_debug_unpack", "chime_bf_n_frames",
     "chime_bf_in_bytes", "chime_bf_out_elems", "chime_bf_launches_per_execute", "chime_bf_destroy",
-    "chime_bf_last_error",
+    "chime_bf_last_error", "chime_bf_update_gains", "chime_bf_update_ew_angles", "chime_bf_update_pointings",
 ]
 
 
@@ -67,6 +67,12 @@ def load_library():
     lib.chime_bf_get_ns_index.argtypes = [vp, vp]
     lib.chime_bf_debug_unpack.restype = ci
     lib.chime_bf_debug_unpack.argtypes = [vp, vp, vp, ctypes.c_size_t, vp]
+    lib.chime_bf_update_gains.restype = ci
+    lib.chime_bf_update_gains.argtypes = [vp, vp, vp]
+    lib.chime_bf_update_ew_angles.restype = ci
+    lib.chime_bf_update_ew_angles.argtypes = [vp, vp, vp]
+    lib.chime_bf_update_pointings.restype = ci
+    lib.chime_bf_update_pointings.argtypes = [vp, vp, ctypes.c_double, vp]
     lib.chime_bf_n_frames.restype = ci
     lib.chime_bf_n_frames.argtypes = [vp]
     lib.chime_bf_in_bytes.restype = ctypes.c_size_t
@@ -155,6 +161,29 @@ class Plan:
         self._check(load_library().chime_bf_execute_host(self._h, _stream_ptr(stream),
                                                          in_u8_host.data_ptr(), out_u8_host.data_ptr()))
         return out_u8_host
+
+    def update_gains(self, gains, stream=None):
+        """chime_bf_update_gains: new per-input gains [n_coarse][2048][2] (None = unit), no plan rebuild."""
+        g = None if gains is None else np.ascontiguousarray(gains, dtype=np.float32)
+        if g is not None and g.size != self.n_coarse * N_INPUT * 2:
+            raise ValueError("gains must have shape [n_coarse][2048][2]")
+        self._check(load_library().chime_bf_update_gains(self._h, _stream_ptr(stream),
+                                                         None if g is None else g.ctypes.data))
+
+    def update_ew_angles(self, ew_angles_deg, stream=None):
+        """chime_bf_update_ew_angles: re-point the 4 E-W beams (tracking beams)."""
+        ew = np.ascontiguousarray(ew_angles_deg, dtype=np.float64)
+        if ew.size != N_EW:
+            raise ValueError("ew_angles must have 4 entries")
+        self._check(load_library().chime_bf_update_ew_angles(self._h, _stream_ptr(stream), ew.ctypes.data))
+
+    def update_pointings(self, f_ref_mhz=0.0, ns_sin_theta=None, stream=None):
+        """chime_bf_update_pointings: re-tile the 256 N-S beams (tunable extent / density)."""
+        s = None if ns_sin_theta is None else np.ascontiguousarray(ns_sin_theta, dtype=np.float64)
+        if s is not None and s.size != N_FEED:
+            raise ValueError("ns_sin_theta must have 256 entries")
+        self._check(load_library().chime_bf_update_pointings(self._h, _stream_ptr(stream), float(f_ref_mhz),
+                                                             None if s is None else s.ctypes.data))
 
     def get_ns_index(self):
         J = np.zeros((self.n_coarse, N_FEED), dtype=np.int32)

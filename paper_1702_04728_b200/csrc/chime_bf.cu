@@ -37,6 +37,12 @@ struct chime_bf_plan {
     int device = 0;
     float scale = 0.f, offset = 0.f, norm = 0.f;
     std::vector<int32_t> J;  // [C][256]
+    // host copies of what the tables are built from (re-plannable without a plan rebuild)
+    std::vector<double> freq;      // [C] MHz
+    std::vector<float> gains;      // [C][2048][2], empty = unit
+    std::vector<double> ns_sin;    // [256] explicit pointings, empty = native grid at fref
+    double ew_deg[4] = {0, 0, 0, 0};
+    double fref = 600.0, d_feed = 0.3048, d_cyl = 22.0;
     float2 *d_wp = nullptr;
     int16_t *d_slot = nullptr;
     int16_t *d_slot_of_m = nullptr;
@@ -88,18 +94,25 @@ bool upload(T **dst, const std::vector<T> &src) {
     return true;
 }
 
-bool build_tables(chime_bf_plan *pl, const chime_bf_params &p, double fref, double d_feed, double d_cyl) {
-    const int C = pl->C, NP = pl->NP, U = pl->U, P = NP / 256;
-    std::vector<float2> wp((size_t)C * 2 * 4 * 4 * 256);
+// First call allocates and copies; later calls (table updates) copy into the same allocation, ordered on `st`.
+template <typename T>
+bool upload_on(T **dst, const std::vector<T> &src, cudaStream_t st) {
+    if (*dst == nullptr) return upload(dst, src);
+    CUDA_TRY(cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+    return true;
+}
+
+// a4: index table J (eq. (1),(2)), compaction of the distinct selected bins into slots.
+bool build_index_tables(chime_bf_plan *pl, cudaStream_t st) {
+    const int C = pl->C, NP = pl->NP, P = NP / 256;
     std::vector<int16_t> slot((size_t)C * NP), slot_of_m((size_t)C * 256);
     pl->J.resize((size_t)C * 256);
     for (int c = 0; c < C; ++c) {
-        const double f = p.freq_mhz ? p.freq_mhz[c] : 800.0 - (double)c * 0.390625;
-        // a4: index table, then compaction of the distinct selected bins into slots
+        const double f = pl->freq[c];
         int32_t *J = &pl->J[(size_t)c * 256];
         for (int m = 0; m < 256; ++m)
-            J[m] = p.ns_sin_theta ? ns_bin_sintheta(NP, f, d_feed, p.ns_sin_theta[m])
-                                  : ns_bin(P, m, f, fref, NP);
+            J[m] = !pl->ns_sin.empty() ? ns_bin_sintheta(NP, f, pl->d_feed, pl->ns_sin[m])
+                                       : ns_bin(P, m, f, pl->fref, NP);
         int16_t *sl = &slot[(size_t)c * NP];
         std::fill(sl, sl + NP, (int16_t)-1);
         for (int m = 0; m < 256; ++m) sl[J[m]] = 0;
@@ -107,6 +120,18 @@ bool build_tables(chime_bf_plan *pl, const chime_bf_params &p, double fref, doub
         for (int j = 0; j < NP; ++j)
             if (sl[j] == 0) sl[j] = ns++;
         for (int m = 0; m < 256; ++m) slot_of_m[(size_t)c * 256 + m] = sl[J[m]];
+    }
+    return upload_on(&pl->d_slot, slot, st) && upload_on(&pl->d_slot_of_m, slot_of_m, st);
+}
+
+// a2 + a5 folded weights (and their tensor-core fragments) from the plan's gains and E-W angles.
+bool build_weight_tables(chime_bf_plan *pl, cudaStream_t st) {
+    const int C = pl->C;
+    const double d_cyl = pl->d_cyl;
+    struct { const float *gains; const double *ew_angles_deg; } p = {pl->gains.empty() ? nullptr : pl->gains.data(), pl->ew_deg};
+    std::vector<float2> wp((size_t)C * 2 * 4 * 4 * 256);
+    for (int c = 0; c < C; ++c) {
+        const double f = pl->freq[c];
         // a2+a5 folded: W'[pol][e][cyl][feed] = exp(-2 pi i f x_cyl sin(phi_e)/c0) * g[pol][cyl][feed]
         for (int e = 0; e < 4; ++e) {
             const double s = std::sin(p.ew_angles_deg[e] * kPi / 180.0);
@@ -157,6 +182,13 @@ bool build_tables(chime_bf_plan *pl, const chime_bf_params &p, double fref, doub
                                 make_uint2((uint32_t)h0 | ((uint32_t)h1 << 16), (uint32_t)l0 | ((uint32_t)l1 << 16));
                         }
     }
+    if (pl->use_mma && !upload_on(&pl->d_bfrag, bfrag, st)) return false;
+    return upload_on(&pl->d_wp, wp, st);
+}
+
+bool build_tables(chime_bf_plan *pl) {
+    const int NP = pl->NP, U = pl->U;
+    if (!build_index_tables(pl, nullptr) || !build_weight_tables(pl, nullptr)) return false;
     std::vector<float2> tw_np(NP), tw_u(U);
     for (int k = 0; k < NP; ++k) {
         const double a = -2.0 * kPi * (double)k / (double)NP;
@@ -177,10 +209,8 @@ bool build_tables(chime_bf_plan *pl, const chime_bf_params &p, double fref, doub
                                       chime2::kSmemBytes));
         CUDA_TRY(cudaFuncSetAttribute(chime3::beamform_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       chime3::kSmemBytesWs));
-        if (!upload(&pl->d_bfrag, bfrag)) return false;
     }
-    return upload(&pl->d_wp, wp) && upload(&pl->d_slot, slot) && upload(&pl->d_slot_of_m, slot_of_m) &&
-           upload(&pl->d_tw_np, tw_np) && upload(&pl->d_tw_u, tw_u);
+    return upload(&pl->d_tw_np, tw_np) && upload(&pl->d_tw_u, tw_u);
 }
 
 template <int P, int RAD>
@@ -312,10 +342,15 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     }
     pl->use_mma = (p.zero_pad == 512 && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
     cudaGetDevice(&pl->device);
-    const double fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
-    const double d_feed = p.feed_spacing_m > 0 ? p.feed_spacing_m : 0.3048;
-    const double d_cyl = p.cyl_spacing_m > 0 ? p.cyl_spacing_m : 22.0;
-    bool ok = build_tables(pl, p, fref, d_feed, d_cyl);
+    pl->fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
+    pl->d_feed = p.feed_spacing_m > 0 ? p.feed_spacing_m : 0.3048;
+    pl->d_cyl = p.cyl_spacing_m > 0 ? p.cyl_spacing_m : 22.0;
+    pl->freq.resize(p.n_coarse);
+    for (int c = 0; c < p.n_coarse; ++c) pl->freq[c] = p.freq_mhz ? p.freq_mhz[c] : 800.0 - (double)c * 0.390625;
+    if (p.gains) pl->gains.assign(p.gains, p.gains + (size_t)p.n_coarse * 2048 * 2);
+    if (p.ns_sin_theta) pl->ns_sin.assign(p.ns_sin_theta, p.ns_sin_theta + 256);
+    for (int e = 0; e < 4; ++e) pl->ew_deg[e] = p.ew_angles_deg[e];
+    bool ok = build_tables(pl);
     ok = ok && prepare_kernel<1, 4>() && prepare_kernel<2, 4>() && prepare_kernel<4, 4>() &&
          prepare_kernel<1, 8>() && prepare_kernel<2, 8>() && prepare_kernel<4, 8>();
     if (!ok) {
@@ -370,6 +405,35 @@ int chime_bf_execute_host(chime_bf_plan *pl, void *stream, const uint8_t *in_hos
         return CHIME_BF_E_CUDA;
     }
     return CHIME_BF_OK;
+}
+
+int chime_bf_update_gains(chime_bf_plan *pl, void *stream, const float *gains) {
+    if (!pl) { set_err("update_gains: null plan"); return CHIME_BF_E_INVALID_ARG; }
+    if (gains) pl->gains.assign(gains, gains + (size_t)pl->C * 2048 * 2);
+    else pl->gains.clear();
+    return build_weight_tables(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
+}
+
+int chime_bf_update_ew_angles(chime_bf_plan *pl, void *stream, const double *ew_angles_deg) {
+    if (!pl || !ew_angles_deg) { set_err("update_ew_angles: null argument"); return CHIME_BF_E_INVALID_ARG; }
+    for (int e = 0; e < 4; ++e) pl->ew_deg[e] = ew_angles_deg[e];
+    return build_weight_tables(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
+}
+
+int chime_bf_update_pointings(chime_bf_plan *pl, void *stream, double f_ref_mhz, const double *ns_sin_theta) {
+    if (!pl) { set_err("update_pointings: null plan"); return CHIME_BF_E_INVALID_ARG; }
+    if (ns_sin_theta) {
+        for (int m = 0; m < 256; ++m)
+            if (!(ns_sin_theta[m] >= -1.0 && ns_sin_theta[m] <= 1.0)) {
+                set_err("update_pointings: ns_sin_theta[%d] outside [-1, 1]", m);
+                return CHIME_BF_E_INVALID_ARG;
+            }
+        pl->ns_sin.assign(ns_sin_theta, ns_sin_theta + 256);
+    } else {
+        pl->ns_sin.clear();
+        if (f_ref_mhz > 0) pl->fref = f_ref_mhz;
+    }
+    return build_index_tables(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
 }
 
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out) {
