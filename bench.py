@@ -8,6 +8,7 @@ coarse channels that rate sustains in real time, 1 channel = 0.8 GB/s).
   python bench.py [--gpus N] [--steps K] [--warmup W]          CUDA arm
   python bench.py --impl reference ...                         oracle arm (CPU, bounded sample)
   python bench.py --workload cfg3 [--chunks 80]                full-band streaming (configs[3]), 1 GPU
+  python bench.py --workload dedisp                            dedispersion kernel (HBM-bound), 1 GPU
 """
 import argparse
 import json
@@ -354,6 +355,59 @@ def run_cfg3(args):
     return 0
 
 
+def run_dedisp(args):
+    """--workload dedisp: the dedispersion kernel on a configs[2]-shaped beam array:
+    uint8 [64 channels][1017 frames][1024 beams][16 fine] = 1.07 GB (>> L2), DM --dm (10: 0.19 s sweep)."""
+    import torch
+
+    import paper_1702_04728_b200 as bf
+    import synth
+
+    torch.cuda.set_device(0)
+    cfg = synth.CONFIGS[2]
+    C, T = cfg["n_coarse"], cfg["n_time"]
+    plan = bf.plan_create_ex(C, freq_mhz=synth.config_freqs(2), n_time=T)
+    g = torch.Generator(device="cuda").manual_seed(synth.config_seed(2))
+    beams = torch.randint(0, 256, plan.out_shape, dtype=torch.uint8, device="cuda", generator=g)
+    dm = args.dm
+    _, n_out = plan.dedisp_delays(dm)
+    out = torch.empty((1024, n_out), dtype=torch.int32, device="cuda")
+    stream = torch.cuda.current_stream()
+    sampler = ClockSampler(0)
+    sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        plan.dedisperse(beams, dm, out_u32=out, stream=stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        plan.dedisperse(beams, dm, out_u32=out, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    clocks = sampler.stop()
+    peaks, peak_kind = measured_peaks()
+    # algorithmic bytes: each (channel, fine) contributes n_out frames of 1024 beams -> C * n_out * 16384 input bytes
+    # (frames outside every track are never needed), plus the uint32 output
+    in_bytes = C * n_out * 1024 * 16
+    nbytes = in_bytes + out.numel() * 4
+    ach = nbytes / (ms * 1e-3) / 1e9
+    line = {
+        "metric": "dedispersion input GB/s (uint8 beams)", "value": in_bytes / (ms * 1e-3) / 1e9, "unit": UNIT,
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8->u32", "data": "synthetic",
+        "config": {"workload": "dedisperse configs[2]-shaped beams: 64 channels x 1017 frames x 1024 beams x 16 fine "
+                               f"(1.07 GB), DM {dm}, {n_out} output samples per beam", "l2": "input >> L2"},
+        "roofline": {"bound": "hbm", "achieved": ach, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
+                     "frac": ach / float(peaks["hbm_gbs"]), "traffic": None, "algorithmic_bytes": nbytes,
+                     "kernel": "chime_dd::dedisperse_kernel", "kernel_ms": ms, "peak_kind": peak_kind},
+        "gpu_launches": args.steps, "clocks": clocks,
+    }
+    print(json.dumps(line))
+    plan.destroy()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -361,12 +415,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="cfg1", choices=["cfg1", "cfg3"],
+    ap.add_argument("--workload", default="cfg1", choices=["cfg1", "cfg3", "dedisp"],
                     help="cfg1 (default, the contract's step) or cfg3 (full-band streaming, 1 GPU)")
     ap.add_argument("--chunks", type=int, default=80, help="cfg3: full-band chunks to stream")
+    ap.add_argument("--dm", type=float, default=10.0, help="dedisp: nominal DM (pc/cm^3)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "dedisp":
+        return run_dedisp(args)
     return run_cfg3(args) if args.workload == "cfg3" else run_cuda(args)
 
 

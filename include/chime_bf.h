@@ -119,6 +119,28 @@ int chime_bf_update_ew_angles(chime_bf_plan *plan, void *cuda_stream, const doub
 int chime_bf_update_pointings(chime_bf_plan *plan, void *cuda_stream, double f_ref_mhz,
                               const double *ns_sin_theta);
 
+/*
+ * Incoherent dedispersion of the beamformer's uint8 output to one nominal DM -- the fourth kernel the paper
+ * proposes (sec. 3.2: "a fourth kernel which will incoherently dedisperse the post-upchannelized
+ * data to a high nominal DM").  Reading F1: with fine-channel frequencies
+ * f(c,g) = f_c + (g - 7.5)*0.390625/16 MHz and output frames of 3*U*2.56 us,
+ *     delay[c][g] = floor( 4148.808 * dm * (f(c,g)^-2 - f_ref^-2) / (3*U*2.56e-6) + 0.5 )   frames,
+ *     D[b][r] = sum_c sum_g beams_u8[c][r + delay[c][g]][b][g],   r = 0 .. n_out-1,  n_out = n_frames - max delay
+ * (exact in uint32; b = ew*256 + ns).
+ *   dm          dispersion measure in pc/cm^3, >= 0
+ *   f_ref_mhz   reference (zero-delay) frequency; <= 0 selects the highest fine-channel frequency of the plan.
+ *               A reference below any fine channel (negative delay) is an error.
+ * chime_bf_dedisp_delays: HOST host_out [C][16] int32 (may be NULL) and HOST *n_out (may be NULL).
+ * chime_bf_dedisperse:    DEVICE beams_u8 [C][n_frames][1024][16] (the layout execute writes), 16-byte aligned;
+ *                         DEVICE out_u32 [1024][n_out]; n_out must be the value dedisp_delays reports (>= 1).
+ *                         Asynchronous on cuda_stream; one kernel launch; uses a plan-owned 64*C-byte table, so
+ *                         one dedisperse call per plan may be in flight at a time.
+ */
+int chime_bf_dedisp_delays(const chime_bf_plan *plan, double dm, double f_ref_mhz, int32_t *host_out,
+                           int *n_out);
+int chime_bf_dedisperse(chime_bf_plan *plan, void *cuda_stream, const uint8_t *beams_u8, double dm,
+                        double f_ref_mhz, uint32_t *out_u32, int n_out);
+
 /* Copy of the clamped N-S bin index table J (eq. (1),(2)): HOST out, [C][256] int32. */
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out);
 

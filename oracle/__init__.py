@@ -181,3 +181,43 @@ def cell(in_u8_cell, f_mhz, gains=None, np_=512, U=128, ew_deg=EW_ANGLES_DEG, fr
     J = ns_index(f_mhz, np_, N_FEED, fref_mhz)
     w = ew_weights(f_mhz, ew_deg, N_CYL, cyl_spacing_m)
     return cell_from_u8(in_u8_cell, gains, J, w, np_, U), J
+
+
+# ---- incoherent dedispersion to a nominal DM (the paper's proposed fourth kernel) --------------
+# Reading F1.  The paper gives no formula; the cold-plasma delay is the textbook one
+# (t = K_DM * DM * f^-2, K_DM = 4.148808 ms GHz^2 cm^3/pc) and is pinned against that constant, not the paper.
+K_DM_MS_GHZ2 = 4.148808
+SAMPLE_S = 2.56e-6          # PAPER.md:37 (Table 1)
+COARSE_MHZ = 0.390625       # 400 MHz / 1024 channels
+
+
+def dedisp_delays(freqs_mhz, dm, U=128, fref_mhz=None, n_fine=N_FINE, n_int=N_INT):
+    """delay[c][g] in output frames (of n_int*U samples): fine channel g of coarse channel c sits at
+    f_c + (g - (n_fine-1)/2) * COARSE_MHZ/n_fine (reading A9: g ascends in frequency); delay relative to fref
+    (default: the highest fine-channel frequency), rounded half up.  Returns (int32 [C][n_fine], max delay)."""
+    f = np.asarray(freqs_mhz, dtype=np.float64)[:, None] + \
+        (np.arange(n_fine, dtype=np.float64)[None, :] - (n_fine - 1) / 2.0) * (COARSE_MHZ / n_fine)
+    if fref_mhz is None or fref_mhz <= 0:
+        fref_mhz = f.max()
+    delay_s = K_DM_MS_GHZ2 * 1e-3 * dm * ((f / 1e3) ** -2 - (fref_mhz / 1e3) ** -2)
+    frames = delay_s / (n_int * U * SAMPLE_S)
+    d = np.floor(frames + 0.5).astype(np.int64)
+    return d.astype(np.int32), int(d.max())
+
+
+def dedisperse(I, delays):
+    """D[b][r] = sum_c sum_g I[c][r + delays[c][g]][b][g], r = 0 .. R - max(delays) - 1.
+    I: [C][R][n_beam][n_fine] (any integer or float dtype); exact in int64 for integer input."""
+    I = np.asarray(I)
+    C, R, B, G = I.shape
+    delays = np.asarray(delays)
+    assert delays.shape == (C, G) and delays.min() >= 0
+    n_out = R - int(delays.max())
+    assert n_out >= 1, "the sweep is longer than the buffer"
+    acc_t = np.int64 if np.issubdtype(I.dtype, np.integer) else np.float64
+    D = np.zeros((B, n_out), dtype=acc_t)
+    for c in range(C):
+        for g in range(G):
+            d = int(delays[c, g])
+            D += I[c, d:d + n_out, :, g].astype(acc_t).T
+    return D

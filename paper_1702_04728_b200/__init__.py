@@ -19,6 +19,7 @@ EXPORTS = [
     "chime_bf_execute_host", "chime_bf_get_ns_index", "chime_bf_debug_unpack", "chime_bf_n_frames",
     "chime_bf_in_bytes", "chime_bf_out_elems", "chime_bf_launches_per_execute", "chime_bf_destroy",
     "chime_bf_last_error", "chime_bf_update_gains", "chime_bf_update_ew_angles", "chime_bf_update_pointings",
+    "chime_bf_dedisp_delays", "chime_bf_dedisperse",
 ]
 
 
@@ -73,6 +74,10 @@ def load_library():
     lib.chime_bf_update_ew_angles.argtypes = [vp, vp, vp]
     lib.chime_bf_update_pointings.restype = ci
     lib.chime_bf_update_pointings.argtypes = [vp, vp, ctypes.c_double, vp]
+    lib.chime_bf_dedisp_delays.restype = ci
+    lib.chime_bf_dedisp_delays.argtypes = [vp, ctypes.c_double, ctypes.c_double, vp, ctypes.POINTER(ci)]
+    lib.chime_bf_dedisperse.restype = ci
+    lib.chime_bf_dedisperse.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp, ci]
     lib.chime_bf_n_frames.restype = ci
     lib.chime_bf_n_frames.argtypes = [vp]
     lib.chime_bf_in_bytes.restype = ctypes.c_size_t
@@ -184,6 +189,29 @@ class Plan:
             raise ValueError("ns_sin_theta must have 256 entries")
         self._check(load_library().chime_bf_update_pointings(self._h, _stream_ptr(stream), float(f_ref_mhz),
                                                              None if s is None else s.ctypes.data))
+
+    def dedisp_delays(self, dm, f_ref_mhz=0.0):
+        """chime_bf_dedisp_delays -> (delay [n_coarse][16] int32, n_out)."""
+        tab = np.zeros((self.n_coarse, N_FINE), dtype=np.int32)
+        n_out = ctypes.c_int(0)
+        self._check(load_library().chime_bf_dedisp_delays(self._h, float(dm), float(f_ref_mhz), tab.ctypes.data,
+                                                          ctypes.byref(n_out)))
+        return tab, n_out.value
+
+    def dedisperse(self, beams_u8, dm, f_ref_mhz=0.0, out_u32=None, stream=None):
+        """chime_bf_dedisperse: uint8 beams [n_coarse][n_frames][4][256][16] -> uint32 [1024][n_out]."""
+        import torch
+        assert beams_u8.is_cuda and beams_u8.dtype == torch.uint8 and beams_u8.is_contiguous()
+        assert beams_u8.numel() == self.out_elems
+        _, n_out = self.dedisp_delays(dm, f_ref_mhz)
+        if n_out < 1:
+            raise ChimeBfError(f"dedisperse: the DM {dm} sweep is longer than the {self.n_frames}-frame buffer")
+        if out_u32 is None:
+            out_u32 = torch.empty((N_BEAM, n_out), dtype=torch.int32, device=beams_u8.device)
+        assert out_u32.is_cuda and out_u32.dtype == torch.int32 and out_u32.numel() == N_BEAM * n_out
+        self._check(load_library().chime_bf_dedisperse(self._h, _stream_ptr(stream), beams_u8.data_ptr(),
+                                                       float(dm), float(f_ref_mhz), out_u32.data_ptr(), n_out))
+        return out_u32
 
     def get_ns_index(self):
         J = np.zeros((self.n_coarse, N_FEED), dtype=np.int32)

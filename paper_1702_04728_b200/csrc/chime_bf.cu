@@ -15,6 +15,7 @@
 #include "beamform_kernel.cuh"
 #include "beamform_mma_kernel.cuh"
 #include "beamform_ws_kernel.cuh"
+#include "dedisperse_kernel.cuh"
 
 namespace {
 
@@ -54,6 +55,7 @@ struct chime_bf_plan {
     // staging for execute_host
     uint8_t *d_stage_in = nullptr;
     uint8_t *d_stage_out = nullptr;
+    int32_t *d_delay = nullptr;   // [C][16] dedispersion delays of the last chime_bf_dedisperse call
 };
 
 namespace {
@@ -210,7 +212,30 @@ bool build_tables(chime_bf_plan *pl) {
         CUDA_TRY(cudaFuncSetAttribute(chime3::beamform_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       chime3::kSmemBytesWs));
     }
+    CUDA_TRY(cudaMalloc((void **)&pl->d_delay, (size_t)pl->C * 16 * sizeof(int32_t)));
     return upload(&pl->d_tw_np, tw_np) && upload(&pl->d_tw_u, tw_u);
+}
+
+// Dispersion delay of fine channel (c, g) relative to f_ref, in output frames (reading F1):
+//   f = f_c + (g - 7.5) * 0.390625/16 MHz,  x = K_DM * DM * (f^-2 - f_ref^-2) / (3 U * 2.56 us),
+//   delay = floor(x + 0.5),  K_DM = 4148.808 s MHz^2 cm^3 / pc.   Returns the largest delay.
+int dedisp_table(const chime_bf_plan *pl, double dm, double fref_mhz, std::vector<int32_t> &tab) {
+    const double fine = 0.390625 / 16.0, tau = 3.0 * (double)pl->U * 2.56e-6;
+    if (!(fref_mhz > 0)) {
+        fref_mhz = 0;
+        for (int c = 0; c < pl->C; ++c) fref_mhz = std::max(fref_mhz, pl->freq[c] + 7.5 * fine);
+    }
+    tab.resize((size_t)pl->C * 16);
+    int mx = 0;
+    for (int c = 0; c < pl->C; ++c)
+        for (int g = 0; g < 16; ++g) {
+            const double f = pl->freq[c] + ((double)g - 7.5) * fine;
+            const double x = 4148.808 * dm * (1.0 / (f * f) - 1.0 / (fref_mhz * fref_mhz)) / tau;
+            const int d = (int)std::floor(x + 0.5);
+            tab[(size_t)c * 16 + g] = d;
+            mx = std::max(mx, d);
+        }
+    return mx;
 }
 
 template <int P, int RAD>
@@ -436,6 +461,55 @@ int chime_bf_update_pointings(chime_bf_plan *pl, void *stream, double f_ref_mhz,
     return build_index_tables(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
 }
 
+int chime_bf_dedisp_delays(const chime_bf_plan *pl, double dm, double f_ref_mhz, int32_t *host_out, int *n_out) {
+    if (!pl || !(dm >= 0)) { set_err("dedisp_delays: bad argument"); return CHIME_BF_E_INVALID_ARG; }
+    std::vector<int32_t> tab;
+    const int mx = dedisp_table(pl, dm, f_ref_mhz, tab);
+    for (int32_t d : tab)
+        if (d < 0) { set_err("dedisp_delays: f_ref below a fine channel (negative delay)"); return CHIME_BF_E_INVALID_ARG; }
+    if (host_out) memcpy(host_out, tab.data(), tab.size() * sizeof(int32_t));
+    if (n_out) *n_out = pl->R - mx;   // complete output samples (<= 0: the sweep is longer than the buffer)
+    return CHIME_BF_OK;
+}
+
+int chime_bf_dedisperse(chime_bf_plan *pl, void *stream, const uint8_t *beams_u8, double dm, double f_ref_mhz,
+                        uint32_t *out_u32, int n_out) {
+    if (!pl || !beams_u8 || !out_u32) { set_err("dedisperse: null argument"); return CHIME_BF_E_INVALID_ARG; }
+    if ((uintptr_t)beams_u8 & 15) { set_err("dedisperse: input must be 16-byte aligned"); return CHIME_BF_E_ALIGNMENT; }
+    std::vector<int32_t> tab((size_t)pl->C * 16);
+    int n_full = 0;
+    const int rc = chime_bf_dedisp_delays(pl, dm, f_ref_mhz, tab.data(), &n_full);
+    if (rc != CHIME_BF_OK) return rc;
+    if (n_full < 1 || n_out != n_full) {
+        set_err("dedisperse: n_out must be n_frames - max delay = %d (got %d)", n_full, n_out);
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(pl->d_delay, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        chime_dd::Params dp;
+        dp.in = reinterpret_cast<const uint32_t *>(beams_u8);
+        dp.delay = pl->d_delay;
+        dp.out = out_u32;
+        dp.C = pl->C;
+        dp.R = pl->R;
+        dp.n_out = n_out;
+        const int bt = 1024 / chime_dd::kBeamsPerCta, tt = (n_out + chime_dd::kTR - 1) / chime_dd::kTR;
+        // fill 148 SMs x 16 resident CTAs: split the channel loop when beams x time tiles are too few
+        int n_split = std::min(pl->C, std::max(1, (148 * 16 + bt * tt - 1) / (bt * tt)));
+        dp.c_per_split = (pl->C + n_split - 1) / n_split;
+        n_split = (pl->C + dp.c_per_split - 1) / dp.c_per_split;
+        if (n_split > 1) e = cudaMemsetAsync(out_u32, 0, (size_t)1024 * n_out * sizeof(uint32_t), st);
+        if (e == cudaSuccess) {
+            dim3 grid(bt, tt, n_split);
+            chime_dd::dedisperse_kernel<<<grid, chime_dd::kThreads, 0, st>>>(dp);
+            e = cudaGetLastError();
+        }
+    }
+    if (e != cudaSuccess) { set_err("dedisperse: %s", cudaGetErrorString(e)); return CHIME_BF_E_CUDA; }
+    return CHIME_BF_OK;
+}
+
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out) {
     if (!plan || !host_out) {
         set_err("get_ns_index: null argument");
@@ -482,6 +556,7 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_bfrag);
     cudaFree(pl->d_stage_in);
     cudaFree(pl->d_stage_out);
+    cudaFree(pl->d_delay);
     delete pl;
 }
 

@@ -1,0 +1,76 @@
+// Incoherent dedispersion of the beamformer output to one nominal DM (the paper's proposed fourth kernel,
+// "a fourth kernel which will incoherently dedisperse the post-upchannelized data to a high
+// nominal DM").  Reading F1 in DESIGN.md:
+//     D[b][r] = sum_c sum_g  I[c][r + delay[c][g]][b][g],      r = 0 .. n_out - 1,
+// I = uint8 intensity codes [C][R][1024 beams][16 fine], delay[c][g] >= 0 in output frames, D exact in uint32
+// (at most 1024 * 16 * 255 < 2^32).  HBM-bound: every input byte is needed exactly once.
+//
+// Mapping: thread <-> (beam, quad of 4 fine channels) loads one 32-bit word per (frame, beam, quad): a warp
+// reads 8 beams x 16 bytes = one 128-byte line per frame.  A CTA of 128 threads owns 32 beams x TR output
+// samples; its accumulators acc[TR] live in registers (static indices).  Each line is read once per fine
+// channel of the quad (4 x, from L1) and once more by the neighbouring time tiles that overlap it by the
+// delay spread inside one coarse channel (from L2); DRAM sees each byte once.  When beams x time tiles alone
+// would not fill the 148 SMs (long sweeps leave few output samples), the channels are split over blockIdx.z
+// and the partial sums meet in the output with integer atomicAdd (exact, order-independent).
+#pragma once
+#include <cstdint>
+
+namespace chime_dd {
+
+constexpr int kTR = 32;          // output samples per thread
+constexpr int kBeamsPerCta = 32; // 128 threads = 32 beams x 4 quads
+constexpr int kThreads = 128;
+
+struct Params {
+    const uint32_t *in;      // [C][R][1024][4] words (4 fine channels per word, little endian)
+    const int32_t *delay;    // [C][16]
+    uint32_t *out;           // [1024][n_out]
+    int C, R, n_out;
+    int c_per_split;         // channels per blockIdx.z slice; > 1 slice: out is pre-zeroed and summed with atomicAdd (exact)
+};
+
+__global__ void __launch_bounds__(kThreads) dedisperse_kernel(const Params p) {
+    const int tid = threadIdx.x;
+    const int q = tid & 3;
+    const int b = blockIdx.x * kBeamsPerCta + (tid >> 2);
+    const int r0 = blockIdx.y * kTR;
+    uint32_t acc[kTR];
+#pragma unroll
+    for (int r = 0; r < kTR; ++r) acc[r] = 0u;
+    const int n_valid = min(kTR, p.n_out - r0);      // ragged last tile
+    const size_t frame_words = 1024 * 4;
+    const int c_lo = blockIdx.z * p.c_per_split, c_hi = min(p.C, c_lo + p.c_per_split);
+#pragma unroll 1
+    for (int c = c_lo; c < c_hi; ++c) {
+        const int4 dl = *reinterpret_cast<const int4 *>(p.delay + c * 16 + 4 * q);
+        const uint32_t *base = p.in + (size_t)c * p.R * frame_words + (size_t)b * 4 + q;
+        const int d[4] = {dl.x, dl.y, dl.z, dl.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t *src = base + (size_t)(r0 + d[j]) * frame_words;
+            if (n_valid == kTR) {
+#pragma unroll
+                for (int r = 0; r < kTR; ++r) acc[r] += (__ldg(src + (size_t)r * frame_words) >> (8 * j)) & 0xFFu;
+            } else {
+#pragma unroll
+                for (int r = 0; r < kTR; ++r)
+                    if (r < n_valid) acc[r] += (__ldg(src + (size_t)r * frame_words) >> (8 * j)) & 0xFFu;
+            }
+        }
+    }
+    // sum the 4 quads of a beam (lanes 4k .. 4k+3), then lane q == 0 .. 3 stores every 4th sample
+#pragma unroll
+    for (int r = 0; r < kTR; ++r) {
+        acc[r] += __shfl_xor_sync(0xFFFFFFFFu, acc[r], 1);
+        acc[r] += __shfl_xor_sync(0xFFFFFFFFu, acc[r], 2);
+    }
+    uint32_t *dst = p.out + (size_t)b * p.n_out + r0;
+#pragma unroll
+    for (int r = 0; r < kTR; ++r)
+        if ((r & 3) == q && r < n_valid) {
+            if (gridDim.z == 1) dst[r] = acc[r];
+            else atomicAdd(dst + r, acc[r]);
+        }
+}
+
+}  // namespace chime_dd

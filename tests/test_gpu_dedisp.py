@@ -1,0 +1,89 @@
+"""GPU parity of the dedispersion kernel (chime_bf_dedisperse; reading F1): delay table and uint32
+sums bit-exact against the oracle on seeded random uint8 beams, ragged tiles included; and the whole chain
+baseband -> beams -> dedispersed series against the oracle chain on a small dispersed pulse."""
+import numpy as np
+import pytest
+import torch
+
+import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def bf():
+    import __graft_entry__ as g
+    g.build()
+    import paper_1702_04728_b200 as bf
+    return bf
+
+
+@pytest.mark.parametrize("C,R,U,dm,step", [(5, 200, 128, 6.0, 100), (3, 77, 256, 9.0, 300), (64, 1017, 128, 40.0, 16),
+                                            (2, 40, 128, 0.0, 1)])
+def test_dedisperse_bit_exact(bf, orc, C, R, U, dm, step):
+    freqs = synth.chime_freqs_mhz(C, step)
+    plan = bf.plan_create_ex(C, freq_mhz=freqs, upchan_len=U, n_time=R * 3 * U)
+    tab, n_out = plan.dedisp_delays(dm)
+    want_tab, mx = orc.dedisp_delays(freqs, dm, U=U)
+    assert np.array_equal(tab, want_tab) and n_out == R - mx and n_out >= 1
+    g = torch.Generator(device="cuda").manual_seed(synth.BASE_SEED + C)
+    beams = torch.randint(0, 256, (C, R, 4, 256, 16), dtype=torch.uint8, device="cuda", generator=g)
+    got = plan.dedisperse(beams, dm).cpu().numpy()
+    hb = beams.cpu().numpy().reshape(C, R, 1024, 16)
+    if C * R > 2000:     # the full cfg2-sized array: oracle on a sample of beams (columns are independent)
+        sel = np.random.default_rng(1).choice(1024, size=48, replace=False)
+        sel[:2] = (0, 1023)
+        want = orc.dedisperse(hb[:, :, sel, :], want_tab)
+        assert np.array_equal(got[sel].astype(np.int64), want)
+    else:
+        assert np.array_equal(got.astype(np.int64), orc.dedisperse(hb, want_tab))
+    if dm > 0:
+        with pytest.raises(bf.ChimeBfError):
+            plan.dedisp_delays(dm, f_ref_mhz=float(freqs.min()))  # reference below the band: negative delays
+    plan.destroy()
+
+
+def test_sweep_longer_than_buffer_is_an_error(bf):
+    plan = bf.plan_create_ex(2, freq_mhz=[800.0, 400.390625], n_time=10 * 384)
+    _, n_out = plan.dedisp_delays(500.0)
+    assert n_out < 1
+    with pytest.raises(bf.ChimeBfError):
+        plan.dedisperse(torch.zeros((2, 10, 4, 256, 16), dtype=torch.uint8, device="cuda"), 500.0)
+
+
+def test_chain_baseband_to_dedispersed_pulse(bf, orc):
+    """8 channels 800 -> 625 MHz, 24 frames, a DM 3 pulse (S/N 20 per channel) from beam (E-W 1, N-S 100):
+    oracle chain (all 192 cells -> uint8 -> dedisperse) vs CUDA chain (execute -> dedisperse)."""
+    C, R, dm = 8, 24, 3.0
+    T = R * 384
+    seed = synth.config_seed(2) + 5
+    freqs = synth.chime_freqs_mhz(C, 64)
+    gains = synth.gains(seed, C, flagged_frac=0.02)
+    m0, e0 = 100, 1
+    s0 = (m0 - 128) * synth.C0 / (256 * 0.3048 * 600e6)
+    b = synth.noise_bytes(seed, C, T)
+    centres = synth.add_pulse(b, seed, freqs, gains=gains, sin_theta=s0, sin_phi=float(np.sin(np.deg2rad(-0.2))),
+                              dm=dm, t0_samples=1000.0)
+    assert centres.max() < T - 640
+    hb = b.numpy()
+    q = np.zeros((C, R, 1024, 16), dtype=np.uint8)
+    for c in range(C):
+        for r in range(R):
+            I, _ = orc.cell(hb[c, 384 * r:384 * (r + 1)], float(freqs[c]), gains=gains[c])
+            q[c, r] = orc.quantize(I).reshape(1024, 16)
+    tab, _ = orc.dedisp_delays(freqs, dm)
+    want = orc.dedisperse(q, tab)
+
+    plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, n_time=T)
+    beams = plan.execute(b.cuda())
+    got = plan.dedisperse(beams, dm).cpu().numpy().astype(np.int64)
+    assert got.shape == want.shape
+    # the uint8 codes may differ by 1 LSB on <= 0.1 % of entries (A15): a sum of 128 codes moves by a few at most
+    assert np.abs(got - want).max() <= 2 and (got != want).mean() < 0.05
+    bpk, rpk = np.unravel_index(want.argmax(), want.shape)
+    assert (bpk // 256, bpk % 256) == (e0, m0) and rpk == int(centres[0]) // 384
+    assert np.unravel_index(got.argmax(), got.shape) == (bpk, rpk)
+    # dedispersion is what makes it stand out: the plain band sum (DM 0) has a lower peak
+    plain = orc.dedisperse(q, np.zeros_like(tab))
+    assert want.max() > plain.max()
+    plan.destroy()
