@@ -7,9 +7,9 @@
 //
 // Mapping: thread <-> (beam, quad of 4 fine channels) loads one 32-bit word per (frame, beam, quad): a warp
 // reads 8 beams x 16 bytes = one 128-byte line per frame.  A CTA of 128 threads owns 32 beams x TR output
-// samples; its accumulators acc[TR] live in registers (static indices).  Each line is read once per fine
-// channel of the quad (4 x, from L1) and once more by the neighbouring time tiles that overlap it by the
-// delay spread inside one coarse channel (from L2); DRAM sees each byte once.  When beams x time tiles alone
+// samples; its accumulators acc[TR] live in registers (static indices).  Each line is read once per distinct
+// delay of the quad (usually one) and once more by the neighbouring time tiles that overlap it by the delay
+// spread inside one coarse channel (from L2); DRAM sees each byte once.  When beams x time tiles alone
 // would not fill the 148 SMs (long sweeps leave few output samples), the channels are split over blockIdx.z
 // and the partial sums meet in the output with integer atomicAdd (exact, order-independent).
 #pragma once
@@ -29,7 +29,7 @@ struct Params {
     int c_per_split;         // channels per blockIdx.z slice; > 1 slice: out is pre-zeroed and summed with atomicAdd (exact)
 };
 
-__global__ void __launch_bounds__(kThreads) dedisperse_kernel(const Params p) {
+__global__ void __launch_bounds__(kThreads, 4) dedisperse_kernel(const Params p) {
     const int tid = threadIdx.x;
     const int q = tid & 3;
     const int b = blockIdx.x * kBeamsPerCta + (tid >> 2);
@@ -44,18 +44,21 @@ __global__ void __launch_bounds__(kThreads) dedisperse_kernel(const Params p) {
     for (int c = c_lo; c < c_hi; ++c) {
         const int4 dl = *reinterpret_cast<const int4 *>(p.delay + c * 16 + 4 * q);
         const uint32_t *base = p.in + (size_t)c * p.R * frame_words + (size_t)b * 4 + q;
-        const int d[4] = {dl.x, dl.y, dl.z, dl.w};
+        // One pass per delay value v of the quad: the lane adds the bytes whose delay is v with dp4a against a
+        // 0/1 byte mask -- every word is loaded once per distinct delay of its quad (once, for most quads),
+        // not once per fine channel.
+        const int v_lo = min(min(dl.x, dl.y), min(dl.z, dl.w)), v_hi = max(max(dl.x, dl.y), max(dl.z, dl.w));
+#pragma unroll 1
+        for (int v = v_lo; v <= v_hi; ++v) {
+            const uint32_t mask = (dl.x == v ? 0x01u : 0u) | (dl.y == v ? 0x0100u : 0u) | (dl.z == v ? 0x010000u : 0u) |
+                                  (dl.w == v ? 0x01000000u : 0u);
+            if (mask == 0u) continue;
+            const uint32_t *src = base + (size_t)(r0 + v) * frame_words;
+            uint32_t w[kTR];   // all TR loads are issued before the first use: 32 x 128 B per warp in flight
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint32_t *src = base + (size_t)(r0 + d[j]) * frame_words;
-            if (n_valid == kTR) {
+            for (int r = 0; r < kTR; ++r) w[r] = (r < n_valid) ? __ldg(src + (size_t)r * frame_words) : 0u;
 #pragma unroll
-                for (int r = 0; r < kTR; ++r) acc[r] += (__ldg(src + (size_t)r * frame_words) >> (8 * j)) & 0xFFu;
-            } else {
-#pragma unroll
-                for (int r = 0; r < kTR; ++r)
-                    if (r < n_valid) acc[r] += (__ldg(src + (size_t)r * frame_words) >> (8 * j)) & 0xFFu;
-            }
+            for (int r = 0; r < kTR; ++r) acc[r] = __dp4a(w[r], mask, acc[r]);
         }
     }
     // sum the 4 quads of a beam (lanes 4k .. 4k+3), then lane q == 0 .. 3 stores every 4th sample
