@@ -392,6 +392,14 @@ def run_dedisp(args):
     in_bytes = C * n_out * 1024 * 16
     nbytes = in_bytes + out.numel() * 4
     ach = nbytes / (ms * 1e-3) / 1e9
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            tj = json.load(f)["dedisp"]
+        if dm == 10.0:
+            traffic = float(tj["dram_bytes_per_launch"])
+    except Exception:
+        pass
     line = {
         "metric": "dedispersion input GB/s (uint8 beams)", "value": in_bytes / (ms * 1e-3) / 1e9, "unit": UNIT,
         "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
@@ -399,7 +407,7 @@ def run_dedisp(args):
         "config": {"workload": "dedisperse configs[2]-shaped beams: 64 channels x 1017 frames x 1024 beams x 16 fine "
                                f"(1.07 GB), DM {dm}, {n_out} output samples per beam", "l2": "input >> L2"},
         "roofline": {"bound": "hbm", "achieved": ach, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
-                     "frac": ach / float(peaks["hbm_gbs"]), "traffic": None, "algorithmic_bytes": nbytes,
+                     "frac": ach / float(peaks["hbm_gbs"]), "traffic": traffic, "algorithmic_bytes": nbytes,
                      "kernel": "chime_dd::dedisperse_kernel", "kernel_ms": ms, "peak_kind": peak_kind},
         "gpu_launches": args.steps, "clocks": clocks,
     }
