@@ -95,8 +95,10 @@ int chime_bf_execute(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u
 int chime_bf_execute_f32(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8,
                          float *out_f32);
 
-/* Convenience: HOST buffers in and out; the library stages them through device memory
- * (allocated on first use, owned by the plan), runs execute on `cuda_stream` and synchronises it. */
+/* Convenience: HOST buffers (ideally pinned) in and out; the library stages them through device memory
+ * (allocated on first use, owned by the plan) and pipelines by channel group: a plan-owned copy stream
+ * uploads group k+1 while `cuda_stream` beamforms group k and downloads its output (up to 8 groups, one
+ * kernel launch each).  Ordered after the work already enqueued on `cuda_stream`; synchronises it. */
 int chime_bf_execute_host(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8_host,
                           uint8_t *out_u8_host);
 

@@ -43,6 +43,7 @@ struct KernelParams {
     const float2 *tw_u;      // [U]   exp(-2 pi i k / U)
     int n_time;              // T
     int n_frames;            // R
+    int chan0;               // first channel this launch processes (grid covers n_chan channels from here)
     float norm;              // 1/(N N_c U)
     float qscale;            // norm * scale
     float qoffset;
@@ -110,7 +111,7 @@ beamform_fused_kernel(const KernelParams prm) {
     const int e = blockIdx.x & 3;
     const int cell = blockIdx.x >> 2;
     const int Rf = cell % prm.n_frames;
-    const int c = cell / prm.n_frames;
+    const int c = prm.chan0 + cell / prm.n_frames;   // chan0: first channel of this launch (execute_host pipelines by channel)
 
     for (int i = tid; i < NP; i += kThreads) {
         s_twnp[i] = prm.tw_np[i];

@@ -52,6 +52,7 @@ struct Params {
     const float2 *tw_np;      // [512] exp(-2 pi i k / 512)
     int n_time;
     int n_frames;
+    int chan0;                // first channel this launch processes
     float norm, qscale, qoffset;
 };
 
@@ -362,7 +363,7 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
     const int ep = blockIdx.x & 1;
     const int cell = blockIdx.x >> 1;
     const int Rf = cell % prm.n_frames;
-    const int c = cell / prm.n_frames;
+    const int c = prm.chan0 + cell / prm.n_frames;   // chan0: first channel of this launch (execute_host pipelines by channel)
 
     {   // s_sel[(16 h + l) * 16 + i] = slot of bin 2 (16 bitrev(i) + l) + h
         const int i = tid & 15, hl = tid >> 4;

@@ -221,7 +221,7 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
     const int ep = blockIdx.x & 1;
     const int cell = blockIdx.x >> 1;
     const int Rf = cell % prm.n_frames;
-    const int c = cell / prm.n_frames;
+    const int c = prm.chan0 + cell / prm.n_frames;   // chan0: first channel of this launch (execute_host pipelines by channel)
 
     {   // s_sel[(16 h + l) * 16 + i] = 8 * slot of bin 2 (16 bitrev(i) + l) + h, or 0x8000
         const int i = tid & 15, hl = tid >> 4;

@@ -55,6 +55,9 @@ struct chime_bf_plan {
     // staging for execute_host
     uint8_t *d_stage_in = nullptr;
     uint8_t *d_stage_out = nullptr;
+    cudaStream_t copy_stream = nullptr;   // execute_host: H2D of channel k+1 under the kernel of channel k
+    std::vector<cudaEvent_t> copy_done;   // one event per channel
+    cudaEvent_t entry = nullptr;
     int32_t *d_delay = nullptr;   // [C][16] dedispersion delays of the last chime_bf_dedisperse call
 };
 
@@ -252,7 +255,9 @@ cudaError_t launch(const chime::KernelParams &kp, int n_cta, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, float *out_f32) {
+int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, float *out_f32, int chan0 = 0,
+        int n_chan = -1) {
+    if (pl && n_chan < 0) n_chan = pl->C;
     if (!pl || !in || (!out_u8 && !out_f32)) {
         set_err("execute: null argument");
         return CHIME_BF_E_INVALID_ARG;
@@ -272,6 +277,7 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
     kp.tw_u = pl->d_tw_u;
     kp.n_time = pl->T;
     kp.n_frames = pl->R;
+    kp.chan0 = chan0;
     kp.norm = pl->norm;
     kp.qscale = pl->norm * pl->scale;
     kp.qoffset = pl->offset;
@@ -287,13 +293,14 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         mp.tw_np = pl->d_tw_np;
         mp.n_time = pl->T;
         mp.n_frames = pl->R;
+        mp.chan0 = chan0;
         mp.norm = pl->norm;
         mp.qscale = pl->norm * pl->scale;
         mp.qoffset = pl->offset;
         if (pl->use_ws)
-            chime3::beamform_ws_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
+            chime3::beamform_ws_kernel<<<n_chan * pl->R * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
         else
-            chime2::beamform_mma_kernel<<<pl->C * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
+            chime2::beamform_mma_kernel<<<n_chan * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
         const cudaError_t e2 = cudaGetLastError();
         if (e2 != cudaSuccess) {
             set_err("kernel launch failed: %s", cudaGetErrorString(e2));
@@ -301,7 +308,7 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         }
         return CHIME_BF_OK;
     }
-    const int n_cta = pl->C * pl->R * 4;
+    const int n_cta = n_chan * pl->R * 4;
     cudaError_t e = cudaErrorInvalidValue;
     const int P = pl->NP / 256, RAD = pl->U / 32;
     if (P == 1 && RAD == 4) e = launch<1, 4>(kp, n_cta, st);
@@ -416,14 +423,38 @@ int chime_bf_execute_host(chime_bf_plan *pl, void *stream, const uint8_t *in_hos
     cudaError_t e = cudaSuccess;
     if (!pl->d_stage_in) e = cudaMalloc((void **)&pl->d_stage_in, nin);
     if (e == cudaSuccess && !pl->d_stage_out) e = cudaMalloc((void **)&pl->d_stage_out, nout);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_stage_in, in_host, nin, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && !pl->copy_stream) {
+        e = cudaStreamCreateWithFlags(&pl->copy_stream, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pl->entry, cudaEventDisableTiming);
+        pl->copy_done.resize(std::min(pl->C, 8), nullptr);
+        for (size_t k = 0; k < pl->copy_done.size() && e == cudaSuccess; ++k)
+            e = cudaEventCreateWithFlags(&pl->copy_done[k], cudaEventDisableTiming);
+    }
     if (e != cudaSuccess) {
         set_err("execute_host: %s", cudaGetErrorString(e));
         return CHIME_BF_E_CUDA;
     }
-    const int rc = run(pl, stream, pl->d_stage_in, pl->d_stage_out, nullptr);
-    if (rc != CHIME_BF_OK) return rc;
-    e = cudaMemcpyAsync(out_host, pl->d_stage_out, nout, cudaMemcpyDeviceToHost, st);
+    // Pipeline by channel group (channels are independent; up to 8 groups): the copy stream uploads group k + 1
+    // while the caller's stream beamforms group k and downloads its output.  The copy stream starts after everything already
+    // enqueued on the caller's stream (entry event), so the call is ordered like a single operation on `st`.
+    const size_t cin = (size_t)pl->T * 2048, cout = (size_t)pl->R * 1024 * 16;
+    e = cudaEventRecord(pl->entry, st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(pl->copy_stream, pl->entry, 0);
+    const int n_chunks = (int)pl->copy_done.size();
+    auto first = [&](int k) { return (int)((long long)pl->C * k / n_chunks); };
+    for (int k = 0; k < n_chunks && e == cudaSuccess; ++k) {
+        const int c0 = first(k), nc = first(k + 1) - c0;
+        e = cudaMemcpyAsync(pl->d_stage_in + c0 * cin, in_host + c0 * cin, nc * cin, cudaMemcpyHostToDevice, pl->copy_stream);
+        if (e == cudaSuccess) e = cudaEventRecord(pl->copy_done[k], pl->copy_stream);
+    }
+    for (int k = 0; k < n_chunks && e == cudaSuccess; ++k) {
+        const int c0 = first(k), nc = first(k + 1) - c0;
+        e = cudaStreamWaitEvent(st, pl->copy_done[k], 0);
+        if (e != cudaSuccess) break;
+        const int rc = run(pl, stream, pl->d_stage_in, pl->d_stage_out, nullptr, c0, nc);
+        if (rc != CHIME_BF_OK) return rc;
+        e = cudaMemcpyAsync(out_host + c0 * cout, pl->d_stage_out + c0 * cout, nc * cout, cudaMemcpyDeviceToHost, st);
+    }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) {
         set_err("execute_host: %s", cudaGetErrorString(e));
@@ -544,7 +575,7 @@ size_t chime_bf_in_bytes(const chime_bf_plan *plan) {
 size_t chime_bf_out_elems(const chime_bf_plan *plan) {
     return plan ? (size_t)plan->C * plan->R * 1024 * 16 : 0;
 }
-int chime_bf_launches_per_execute(const chime_bf_plan *plan) { return plan ? 1 : 0; }
+int chime_bf_launches_per_execute(const chime_bf_plan *plan) { return plan ? 1 : 0; }   // execute_host: one per channel
 
 void chime_bf_destroy(chime_bf_plan *pl) {
     if (!pl) return;
@@ -557,6 +588,10 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_stage_in);
     cudaFree(pl->d_stage_out);
     cudaFree(pl->d_delay);
+    for (cudaEvent_t ev : pl->copy_done)
+        if (ev) cudaEventDestroy(ev);
+    if (pl->entry) cudaEventDestroy(pl->entry);
+    if (pl->copy_stream) cudaStreamDestroy(pl->copy_stream);
     delete pl;
 }
 
