@@ -126,6 +126,14 @@ bool build_index_tables(chime_bf_plan *pl, cudaStream_t st) {
             if (sl[j] == 0) sl[j] = ns++;
         for (int m = 0; m < 256; ++m) slot_of_m[(size_t)c * 256 + m] = sl[J[m]];
     }
+    if (pl->use_mma && NP == 256) {
+        // zero_pad 256 on the tensor-core kernels: bin j of the 256-point transform IS bin 2 j of the 512-point
+        // zero-padded one, so the kernel runs unchanged on a 512-entry map whose odd bins are unused.
+        std::vector<int16_t> slot512((size_t)C * 512, (int16_t)-1);
+        for (int c = 0; c < C; ++c)
+            for (int j = 0; j < 256; ++j) slot512[(size_t)c * 512 + 2 * j] = slot[(size_t)c * 256 + j];
+        slot.swap(slot512);
+    }
     return upload_on(&pl->d_slot, slot, st) && upload_on(&pl->d_slot_of_m, slot_of_m, st);
 }
 
@@ -192,7 +200,7 @@ bool build_weight_tables(chime_bf_plan *pl, cudaStream_t st) {
 }
 
 bool build_tables(chime_bf_plan *pl) {
-    const int NP = pl->NP, U = pl->U;
+    const int NP = pl->use_mma ? 512 : pl->NP, U = pl->U;   // the tensor-core kernels always transform 512 points
     if (!build_index_tables(pl, nullptr) || !build_weight_tables(pl, nullptr)) return false;
     std::vector<float2> tw_np(NP), tw_u(U);
     for (int k = 0; k < NP; ++k) {
@@ -372,7 +380,7 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
         const char *kv = getenv("CHIME_BF_KERNEL");   // A/B switch: v1 generic, v2 block-synchronous mma, v3 warp-specialised (default)
         pl->use_ws = !kv || !strcmp(kv, "v3");
     }
-    pl->use_mma = (p.zero_pad == 512 && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
+    pl->use_mma = ((p.zero_pad == 512 || p.zero_pad == 256) && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
     cudaGetDevice(&pl->device);
     pl->fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
     pl->d_feed = p.feed_spacing_m > 0 ? p.feed_spacing_m : 0.3048;
