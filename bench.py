@@ -173,7 +173,7 @@ def run_cuda(args):
     chan0, _ = weak_scaling_shard(C, rank)
     freqs = synth.chime_freqs_mhz(C, 1, k0=chan0)
     gains = synth.gains(seed + 1000 * rank, C, flagged_frac=cfg["flagged"])
-    plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, zero_pad=512, upchan_len=128, n_time=T)
+    plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, zero_pad=args.zero_pad, upchan_len=args.upchan, n_time=T)
     d_in = synth.noise_bytes(seed, C, T, device="cuda", chan0=chan0)
     d_out = torch.empty(plan.out_shape, dtype=torch.uint8, device="cuda")
     h_in = d_in.cpu().pin_memory()
@@ -246,14 +246,19 @@ def run_cuda(args):
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     fp32_peak = N_SM * LANES * 2 * sm_mhz * 1e6 / 1e12
     chan_samples = C * T
-    ach = FFT_FLOPS * chan_samples / (kern_ms * 1e-3) / 1e12
+    import math
+    # nominal FFT flops per (channel, sample): 8 rows x 5 NP log2 NP (N-S) + 2048 series x 5 log2 U (time)
+    fft_flops = 8 * 5.0 * args.zero_pad * math.log2(args.zero_pad) + 2048 * 5.0 * math.log2(args.upchan)
+    assert (args.zero_pad, args.upchan) != (512, 128) or fft_flops == FFT_FLOPS
+    ach = fft_flops * chan_samples / (kern_ms * 1e-3) / 1e12
     hbm_peak = float(peaks["hbm_gbs"])
     hbm_ach = (in_bytes + out_bytes) / (kern_ms * 1e-3) / 1e9
     traffic, traffic_src = None, None
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             tj = json.load(f)
-        traffic, traffic_src = float(tj["dram_bytes_per_launch"]), tj["source"]
+        if args.zero_pad == 512 and args.upchan == 128:     # the profile is of the default setting
+            traffic, traffic_src = float(tj["dram_bytes_per_launch"]), tj["source"]
     except Exception:
         pass
     line = {
@@ -263,7 +268,7 @@ def run_cuda(args):
         "channels_realtime": gbs / GBS_PER_CHANNEL,
         "realtime_fraction_full_band": gbs / (1024 * GBS_PER_CHANNEL),
         "config": {"workload": "configs[1] single node load per GPU: 4 coarse channels x 49152 samples x "
-                               "2048 inputs, zero_pad 512, upchan 128, random gains, 2% flagged",
+                               f"2048 inputs, zero_pad {args.zero_pad}, upchan {args.upchan}, random gains, 2% flagged",
                    "in_bytes_per_step": in_bytes, "out_bytes_per_step": out_bytes,
                    "l2": "input (403 MB) larger than L2 (126 MB); no flush needed",
                    "parallelism": f"channel-sharded x{world}, no collective"},
@@ -271,8 +276,9 @@ def run_cuda(args):
                      "frac": ach / fp32_peak, "traffic": traffic,
                      "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
                      "traffic_source": traffic_src, "algorithmic_bytes": in_bytes + out_bytes,
-                     "kernel": "chime3::beamform_ws_kernel", "kernel_ms": kern_ms,
-                     "flops_per_chan_sample": FFT_FLOPS,
+                     "kernel": ("chime3::beamform_ws_kernel" if args.upchan == 128 and args.zero_pad in (256, 512)
+                                else "chime::beamform_fused_kernel"), "kernel_ms": kern_ms,
+                     "flops_per_chan_sample": fft_flops,
                      "note": f"FP32 peak = 148 SM x 128 lanes x 2 x {sm_mhz:.0f} MHz ({peak_kind} sm_max_mhz); "
                              "nominal FFT flops (5 n log2 n) per BASELINE north_star",
                      "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
@@ -426,6 +432,9 @@ def main():
     ap.add_argument("--workload", default="cfg1", choices=["cfg1", "cfg3", "dedisp"],
                     help="cfg1 (default, the contract's step) or cfg3 (full-band streaming, 1 GPU)")
     ap.add_argument("--chunks", type=int, default=80, help="cfg3: full-band chunks to stream")
+    ap.add_argument("--zero-pad", type=int, default=512, choices=[256, 512, 1024],
+                    help="cfg1: padded N-S length (512 = the paper's and the contract's setting)")
+    ap.add_argument("--upchan", type=int, default=128, choices=[128, 256], help="cfg1: up-channelisation length")
     ap.add_argument("--dm", type=float, default=10.0, help="dedisp: nominal DM (pc/cm^3)")
     args = ap.parse_args()
     if args.impl == "reference":

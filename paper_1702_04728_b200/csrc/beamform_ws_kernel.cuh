@@ -363,11 +363,13 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
 #pragma unroll
                 for (int g = 0; g < 16; ++g) fb[sl * 17 + g] = acc[g] * prm.norm;
                 bar_sync(BAR_CONS, kCThreads);
-                const int s = s_slot_of_m[sl];
+                const int s = s_slot_of_m[sl];   // < 0: beam sl belongs to the other pass (zero_pad 1024 runs two)
                 float4 *dst = reinterpret_cast<float4 *>(prm.out_f32 + out_base + (size_t)sl * 16);
+                if (s >= 0) {
 #pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    dst[k] = make_float4(fb[s * 17 + 4 * k], fb[s * 17 + 4 * k + 1], fb[s * 17 + 4 * k + 2], fb[s * 17 + 4 * k + 3]);
+                    for (int k = 0; k < 4; ++k)
+                        dst[k] = make_float4(fb[s * 17 + 4 * k], fb[s * 17 + 4 * k + 1], fb[s * 17 + 4 * k + 2], fb[s * 17 + 4 * k + 3]);
+                }
             } else {
                 uint32_t q[4];
 #pragma unroll
@@ -385,7 +387,7 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
                 qb[sl] = make_uint4(q[0], q[1], q[2], q[3]);
                 bar_sync(BAR_CONS, kCThreads);
                 const int s = s_slot_of_m[sl];
-                reinterpret_cast<uint4 *>(prm.out_u8 + out_base)[sl] = qb[s];
+                if (s >= 0) reinterpret_cast<uint4 *>(prm.out_u8 + out_base)[sl] = qb[s];
             }
             bar_sync(BAR_CONS, kCThreads);
         }

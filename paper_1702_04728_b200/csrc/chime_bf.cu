@@ -52,6 +52,7 @@ struct chime_bf_plan {
     uint2 *d_bfrag = nullptr;  // tensor-core B fragments of the folded weights (zero_pad 512, upchan 128 path)
     bool use_mma = false;
     bool use_ws = false;       // warp-specialised variant of the tensor-core path (default)
+    int n_pass = 1;            // zero_pad 1024 on the tensor-core kernel: two passes (even / odd bins), see build_index_tables
     // staging for execute_host
     uint8_t *d_stage_in = nullptr;
     uint8_t *d_stage_out = nullptr;
@@ -126,6 +127,28 @@ bool build_index_tables(chime_bf_plan *pl, cudaStream_t st) {
             if (sl[j] == 0) sl[j] = ns++;
         for (int m = 0; m < 256; ++m) slot_of_m[(size_t)c * 256 + m] = sl[J[m]];
     }
+    if (pl->use_mma && NP == 1024) {
+        // zero_pad 1024 as TWO passes of the 512-point kernel: X[j] = sum_n v[n] W_1024^{n j}.
+        //   pass 0, j even:  bin j/2 of the 512-point transform of v[n]
+        //   pass 1, j odd:   bin (j-1)/2 of the 512-point transform of v[n] W_1024^n  (the factor is folded into
+        //                    the pass's E-W weights, build_weight_tables)
+        // Every beam has one bin, hence one pass; the other pass's slot_of_m is -1 and its epilogue skips the beam.
+        std::vector<int16_t> s2((size_t)2 * C * 512, (int16_t)-1), m2((size_t)2 * C * 256, (int16_t)-1);
+        for (int pass = 0; pass < 2; ++pass)
+            for (int c = 0; c < C; ++c) {
+                int16_t *sl = &s2[((size_t)pass * C + c) * 512];
+                const int32_t *J = &pl->J[(size_t)c * 256];
+                for (int m = 0; m < 256; ++m)
+                    if ((J[m] & 1) == pass) sl[J[m] >> 1] = 0;
+                int16_t ns = 0;
+                for (int j = 0; j < 512; ++j)
+                    if (sl[j] == 0) sl[j] = ns++;
+                for (int m = 0; m < 256; ++m)
+                    if ((J[m] & 1) == pass) m2[((size_t)pass * C + c) * 256 + m] = sl[J[m] >> 1];
+            }
+        slot.swap(s2);
+        slot_of_m.swap(m2);
+    }
     if (pl->use_mma && NP == 256) {
         // zero_pad 256 on the tensor-core kernels: bin j of the 256-point transform IS bin 2 j of the 512-point
         // zero-padded one, so the kernel runs unchanged on a 512-entry map whose odd bins are unused.
@@ -171,27 +194,34 @@ bool build_weight_tables(chime_bf_plan *pl, cudaStream_t st) {
     // zero, so only lanes 0..15 are stored.
     std::vector<uint2> bfrag;
     if (pl->use_mma) {
-        bfrag.resize((size_t)C * 2 * 2 * 256 * 16);
+        const size_t per_pass = (size_t)C * 2 * 2 * 256 * 16;
+        bfrag.resize(per_pass * pl->n_pass);
         auto split = [](float v, uint16_t &hi, uint16_t &lo) {
             const __half h = __float2half_rn(v);
             const __half l = __float2half_rn(v - __half2float(h));
             memcpy(&hi, &h, 2);
             memcpy(&lo, &l, 2);
         };
+        for (int pass = 0; pass < pl->n_pass; ++pass)
         for (int c = 0; c < C; ++c)
             for (int pol = 0; pol < 2; ++pol)
                 for (int ep = 0; ep < 2; ++ep)
                     for (int n = 0; n < 256; ++n)
                         for (int lane = 0; lane < 16; ++lane) {
                             const int g = lane >> 2, cyl = lane & 3, e = 2 * ep + (g >> 1), ro = g & 1;
-                            const float2 w = wp[((((size_t)c * 2 + pol) * 4 + e) * 4 + cyl) * 256 + n];
+                            float2 w = wp[((((size_t)c * 2 + pol) * 4 + e) * 4 + cyl) * 256 + n];
+                            if (pass == 1) {   // odd bins of the 1024-point transform: v[n] W_1024^n (double, then float)
+                                const double a = -2.0 * kPi * (double)n / 1024.0, cr = std::cos(a), ci = std::sin(a);
+                                w = make_float2((float)((double)w.x * cr - (double)w.y * ci),
+                                                (float)((double)w.x * ci + (double)w.y * cr));
+                            }
                             // output re: k=(cyl,re)-> wr, k=(cyl,im)-> -wi ; output im: wi, wr
                             const float k0 = 512.0f * (ro == 0 ? w.x : w.y);
                             const float k1 = 512.0f * (ro == 0 ? -w.y : w.x);
                             uint16_t h0, l0, h1, l1;
                             split(k0, h0, l0);
                             split(k1, h1, l1);
-                            bfrag[((((size_t)c * 2 + pol) * 2 + ep) * 256 + n) * 16 + lane] =
+                            bfrag[pass * per_pass + ((((size_t)c * 2 + pol) * 2 + ep) * 256 + n) * 16 + lane] =
                                 make_uint2((uint32_t)h0 | ((uint32_t)h1 << 16), (uint32_t)l0 | ((uint32_t)l1 << 16));
                         }
     }
@@ -305,10 +335,15 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         mp.norm = pl->norm;
         mp.qscale = pl->norm * pl->scale;
         mp.qoffset = pl->offset;
-        if (pl->use_ws)
-            chime3::beamform_ws_kernel<<<n_chan * pl->R * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
-        else
-            chime2::beamform_mma_kernel<<<n_chan * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
+        for (int pass = 0; pass < pl->n_pass; ++pass) {
+            mp.bfrag = pl->d_bfrag + (size_t)pass * pl->C * 2 * 2 * 256 * 16;
+            mp.slot = pl->d_slot + (size_t)pass * pl->C * 512;
+            mp.slot_of_m = pl->d_slot_of_m + (size_t)pass * pl->C * 256;
+            if (pl->use_ws)
+                chime3::beamform_ws_kernel<<<n_chan * pl->R * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
+            else
+                chime2::beamform_mma_kernel<<<n_chan * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
+        }
         const cudaError_t e2 = cudaGetLastError();
         if (e2 != cudaSuccess) {
             set_err("kernel launch failed: %s", cudaGetErrorString(e2));
@@ -380,7 +415,8 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
         const char *kv = getenv("CHIME_BF_KERNEL");   // A/B switch: v1 generic, v2 block-synchronous mma, v3 warp-specialised (default)
         pl->use_ws = !kv || !strcmp(kv, "v3");
     }
-    pl->use_mma = ((p.zero_pad == 512 || p.zero_pad == 256) && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
+    pl->n_pass = (p.zero_pad == 1024 && p.upchan_len == 128 && pl->use_ws) ? 2 : 1;
+    pl->use_mma = ((p.zero_pad == 512 || p.zero_pad == 256 || pl->n_pass == 2) && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
     cudaGetDevice(&pl->device);
     pl->fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
     pl->d_feed = p.feed_spacing_m > 0 ? p.feed_spacing_m : 0.3048;
@@ -583,7 +619,7 @@ size_t chime_bf_in_bytes(const chime_bf_plan *plan) {
 size_t chime_bf_out_elems(const chime_bf_plan *plan) {
     return plan ? (size_t)plan->C * plan->R * 1024 * 16 : 0;
 }
-int chime_bf_launches_per_execute(const chime_bf_plan *plan) { return plan ? 1 : 0; }   // execute_host: one per channel
+int chime_bf_launches_per_execute(const chime_bf_plan *plan) { return plan ? plan->n_pass : 0; }   // execute_host: one per channel
 
 void chime_bf_destroy(chime_bf_plan *pl) {
     if (!pl) return;

@@ -44,7 +44,7 @@ def _check(orc, plan, d_in, hb, freqs, gains, cells, NP, U, ew_deg, fref=600.0, 
     return out_u8
 
 
-@pytest.mark.parametrize("NP,U", [(512, 128), (1024, 256)])
+@pytest.mark.parametrize("NP,U", [(512, 128), (1024, 128), (256, 128), (1024, 256)])
 def test_update_tables_match_oracle_and_fresh_plan(bf, orc, NP, U):
     C, T = 2, 2 * 3 * U
     seed = synth.config_seed(1) + 17
