@@ -97,8 +97,8 @@ int chime_bf_execute_f32(chime_bf_plan *plan, void *cuda_stream, const uint8_t *
 
 /* Convenience: HOST buffers (ideally pinned) in and out; the library stages them through device memory
  * (allocated on first use, owned by the plan) and pipelines by channel group: a plan-owned copy stream
- * uploads group k+1 while `cuda_stream` beamforms group k and downloads its output (up to 8 groups, one
- * kernel launch each).  Ordered after the work already enqueued on `cuda_stream`; synchronises it. */
+ * uploads chunk k+1 while `cuda_stream` beamforms chunk k and downloads its output (up to 8 chunks: channel
+ * groups, or frame ranges of each channel when there are fewer than 8 channels; one kernel launch each).  Ordered after the work already enqueued on `cuda_stream`; synchronises it. */
 int chime_bf_execute_host(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8_host,
                           uint8_t *out_u8_host);
 

@@ -44,6 +44,7 @@ struct KernelParams {
     int n_time;              // T
     int n_frames;            // R
     int chan0;               // first channel this launch processes (grid covers n_chan channels from here)
+    int frame0, n_frames_launch;   // frame range of this launch within each channel
     float norm;              // 1/(N N_c U)
     float qscale;            // norm * scale
     float qoffset;
@@ -110,8 +111,9 @@ beamform_fused_kernel(const KernelParams prm) {
     const int lane = tid & 31, warp = tid >> 5;
     const int e = blockIdx.x & 3;
     const int cell = blockIdx.x >> 2;
-    const int Rf = cell % prm.n_frames;
-    const int c = prm.chan0 + cell / prm.n_frames;   // chan0: first channel of this launch (execute_host pipelines by channel)
+    // a launch covers frames [frame0, frame0 + n_frames_launch) of channels chan0 ... (execute_host pipelines)
+    const int Rf = prm.frame0 + cell % prm.n_frames_launch;
+    const int c = prm.chan0 + cell / prm.n_frames_launch;
 
     for (int i = tid; i < NP; i += kThreads) {
         s_twnp[i] = prm.tw_np[i];

@@ -53,6 +53,7 @@ struct Params {
     int n_time;
     int n_frames;
     int chan0;                // first channel this launch processes
+    int frame0, n_frames_launch;   // frame range of this launch within each channel
     float norm, qscale, qoffset;
 };
 
@@ -362,8 +363,9 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_mma_kernel(const Params 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ep = blockIdx.x & 1;
     const int cell = blockIdx.x >> 1;
-    const int Rf = cell % prm.n_frames;
-    const int c = prm.chan0 + cell / prm.n_frames;   // chan0: first channel of this launch (execute_host pipelines by channel)
+    // a launch covers frames [frame0, frame0 + n_frames_launch) of channels chan0 ... (execute_host pipelines)
+    const int Rf = prm.frame0 + cell % prm.n_frames_launch;
+    const int c = prm.chan0 + cell / prm.n_frames_launch;
 
     {   // s_sel[(16 h + l) * 16 + i] = slot of bin 2 (16 bitrev(i) + l) + h
         const int i = tid & 15, hl = tid >> 4;

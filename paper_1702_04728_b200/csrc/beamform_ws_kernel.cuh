@@ -220,8 +220,9 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ep = blockIdx.x & 1;
     const int cell = blockIdx.x >> 1;
-    const int Rf = cell % prm.n_frames;
-    const int c = prm.chan0 + cell / prm.n_frames;   // chan0: first channel of this launch (execute_host pipelines by channel)
+    // a launch covers frames [frame0, frame0 + n_frames_launch) of channels chan0 ... (execute_host pipelines)
+    const int Rf = prm.frame0 + cell % prm.n_frames_launch;
+    const int c = prm.chan0 + cell / prm.n_frames_launch;
 
     {   // s_sel[(16 h + l) * 16 + i] = 8 * slot of bin 2 (16 bitrev(i) + l) + h, or 0x8000
         const int i = tid & 15, hl = tid >> 4;

@@ -59,6 +59,7 @@ struct chime_bf_plan {
     cudaStream_t copy_stream = nullptr;   // execute_host: H2D of channel k+1 under the kernel of channel k
     std::vector<cudaEvent_t> copy_done;   // one event per channel
     cudaEvent_t entry = nullptr;
+    int host_parts = 1;                   // execute_host: frame ranges per channel
     int32_t *d_delay = nullptr;   // [C][16] dedispersion delays of the last chime_bf_dedisperse call
 };
 
@@ -294,8 +295,9 @@ cudaError_t launch(const chime::KernelParams &kp, int n_cta, cudaStream_t st) {
 }
 
 int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, float *out_f32, int chan0 = 0,
-        int n_chan = -1) {
+        int n_chan = -1, int frame0 = 0, int n_fr = -1) {
     if (pl && n_chan < 0) n_chan = pl->C;
+    if (pl && n_fr < 0) n_fr = pl->R;
     if (!pl || !in || (!out_u8 && !out_f32)) {
         set_err("execute: null argument");
         return CHIME_BF_E_INVALID_ARG;
@@ -316,6 +318,8 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
     kp.n_time = pl->T;
     kp.n_frames = pl->R;
     kp.chan0 = chan0;
+    kp.frame0 = frame0;
+    kp.n_frames_launch = n_fr;
     kp.norm = pl->norm;
     kp.qscale = pl->norm * pl->scale;
     kp.qoffset = pl->offset;
@@ -332,6 +336,8 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         mp.n_time = pl->T;
         mp.n_frames = pl->R;
         mp.chan0 = chan0;
+        mp.frame0 = frame0;
+        mp.n_frames_launch = n_fr;
         mp.norm = pl->norm;
         mp.qscale = pl->norm * pl->scale;
         mp.qoffset = pl->offset;
@@ -340,9 +346,9 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
             mp.slot = pl->d_slot + (size_t)pass * pl->C * 512;
             mp.slot_of_m = pl->d_slot_of_m + (size_t)pass * pl->C * 256;
             if (pl->use_ws)
-                chime3::beamform_ws_kernel<<<n_chan * pl->R * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
+                chime3::beamform_ws_kernel<<<n_chan * n_fr * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
             else
-                chime2::beamform_mma_kernel<<<n_chan * pl->R * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
+                chime2::beamform_mma_kernel<<<n_chan * n_fr * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
         }
         const cudaError_t e2 = cudaGetLastError();
         if (e2 != cudaSuccess) {
@@ -351,7 +357,7 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         }
         return CHIME_BF_OK;
     }
-    const int n_cta = n_chan * pl->R * 4;
+    const int n_cta = n_chan * n_fr * 4;
     cudaError_t e = cudaErrorInvalidValue;
     const int P = pl->NP / 256, RAD = pl->U / 32;
     if (P == 1 && RAD == 4) e = launch<1, 4>(kp, n_cta, st);
@@ -470,7 +476,9 @@ int chime_bf_execute_host(chime_bf_plan *pl, void *stream, const uint8_t *in_hos
     if (e == cudaSuccess && !pl->copy_stream) {
         e = cudaStreamCreateWithFlags(&pl->copy_stream, cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pl->entry, cudaEventDisableTiming);
-        pl->copy_done.resize(std::min(pl->C, 8), nullptr);
+        // up to 8 chunks: whole channels if there are at least 8, else every channel in 8 / C frame ranges
+        pl->host_parts = pl->C >= 8 ? 1 : std::max(1, std::min(pl->R, 8 / pl->C));
+        pl->copy_done.resize(pl->host_parts == 1 ? std::min(pl->C, 8) : pl->C * pl->host_parts, nullptr);
         for (size_t k = 0; k < pl->copy_done.size() && e == cudaSuccess; ++k)
             e = cudaEventCreateWithFlags(&pl->copy_done[k], cudaEventDisableTiming);
     }
@@ -484,20 +492,40 @@ int chime_bf_execute_host(chime_bf_plan *pl, void *stream, const uint8_t *in_hos
     const size_t cin = (size_t)pl->T * 2048, cout = (size_t)pl->R * 1024 * 16;
     e = cudaEventRecord(pl->entry, st);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(pl->copy_stream, pl->entry, 0);
+    // chunk k = (channel range, frame range): whole channels when C >= 8, else each channel in `parts` frame ranges
     const int n_chunks = (int)pl->copy_done.size();
-    auto first = [&](int k) { return (int)((long long)pl->C * k / n_chunks); };
+    const int parts = pl->host_parts;
+    const size_t fin = (size_t)3 * pl->U * 2048, fout = (size_t)1024 * 16;   // bytes per frame in / out
+    auto chunk = [&](int k, int &c0, int &nc, int &f0, int &nf) {
+        if (parts == 1) {
+            c0 = (int)((long long)pl->C * k / n_chunks);
+            nc = (int)((long long)pl->C * (k + 1) / n_chunks) - c0;
+            f0 = 0;
+            nf = pl->R;
+        } else {
+            c0 = k / parts;
+            nc = 1;
+            f0 = (int)((long long)pl->R * (k % parts) / parts);
+            nf = (int)((long long)pl->R * (k % parts + 1) / parts) - f0;
+        }
+    };
     for (int k = 0; k < n_chunks && e == cudaSuccess; ++k) {
-        const int c0 = first(k), nc = first(k + 1) - c0;
-        e = cudaMemcpyAsync(pl->d_stage_in + c0 * cin, in_host + c0 * cin, nc * cin, cudaMemcpyHostToDevice, pl->copy_stream);
+        int c0, nc, f0, nf;
+        chunk(k, c0, nc, f0, nf);
+        const size_t off = c0 * cin + f0 * fin;
+        e = cudaMemcpyAsync(pl->d_stage_in + off, in_host + off, nc == 1 ? nf * fin : nc * cin, cudaMemcpyHostToDevice,
+                            pl->copy_stream);
         if (e == cudaSuccess) e = cudaEventRecord(pl->copy_done[k], pl->copy_stream);
     }
     for (int k = 0; k < n_chunks && e == cudaSuccess; ++k) {
-        const int c0 = first(k), nc = first(k + 1) - c0;
+        int c0, nc, f0, nf;
+        chunk(k, c0, nc, f0, nf);
         e = cudaStreamWaitEvent(st, pl->copy_done[k], 0);
         if (e != cudaSuccess) break;
-        const int rc = run(pl, stream, pl->d_stage_in, pl->d_stage_out, nullptr, c0, nc);
+        const int rc = run(pl, stream, pl->d_stage_in, pl->d_stage_out, nullptr, c0, nc, f0, nf);
         if (rc != CHIME_BF_OK) return rc;
-        e = cudaMemcpyAsync(out_host + c0 * cout, pl->d_stage_out + c0 * cout, nc * cout, cudaMemcpyDeviceToHost, st);
+        const size_t off = c0 * cout + f0 * fout;
+        e = cudaMemcpyAsync(out_host + off, pl->d_stage_out + off, nc == 1 ? nf * fout : nc * cout, cudaMemcpyDeviceToHost, st);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) {

@@ -118,13 +118,20 @@ def test_degenerate_inputs(bf, orc):
     assert int(q.max()) == 255 and int(q.min()) == 128
 
 
-def test_execute_host_matches_device(bf):
-    T = 768
-    plan = bf.plan_create_ex(2, n_time=T)
-    b = synth.noise_bytes(11, 2, T)
+@pytest.mark.parametrize("C,frames,NP,U", [(2, 2, 512, 128), (3, 5, 1024, 128), (9, 2, 1024, 256), (1, 1, 256, 128),
+                                            (13, 3, 512, 128)])
+def test_execute_host_matches_device(bf, C, frames, NP, U):
+    """execute_host pipelines H2D / kernels / D2H over up to 8 chunks (channel groups, or frame ranges of each
+    channel when there are fewer than 8 channels): the result must be the device path's, bit for bit."""
+    T = frames * 3 * U
+    plan = bf.plan_create_ex(C, zero_pad=NP, upchan_len=U, n_time=T, gains=synth.gains(5, C))
+    b = synth.noise_bytes(11, C, T)
     ref = plan.execute(b.cuda()).cpu()
     out = plan.execute_host(b.pin_memory())
     assert torch.equal(ref, out.reshape(ref.shape))
+    out2 = plan.execute_host(b.pin_memory())          # second call re-uses the staging buffers and events
+    assert torch.equal(ref, out2.reshape(ref.shape))
+    plan.destroy()
 
 
 def test_cfg1_full_size_sampled(bf, orc):
