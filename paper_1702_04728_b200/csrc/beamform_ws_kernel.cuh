@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
 
     if (warp >= kConsumerWarps) {
         // ======================================= PRODUCERS =======================================
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
         const int ptid = tid - kCThreads;
 #pragma unroll 1
         for (int blk = 0; blk < 6; ++blk) {
@@ -294,7 +294,7 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
         }
     } else {
         // ======================================= CONSUMERS =======================================
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 168;");
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 176;");
         const int h = lane >> 4, l = lane & 15;
         const int rx = rw & 7, xx = h ? 0 : rx;   // rows rw, rw + 8, rw + 16, rw + 24 share the swizzle
         const int rd = (((l >> 1) ^ rx) << 4) | ((l & 1) << 3);
