@@ -141,46 +141,56 @@ __device__ __forceinline__ void phase_b_2rows(unsigned char *S, const int rowA, 
         a0[k] = *reinterpret_cast<const float2 *>(S + (ra0 + 128 * k));
         a1[k] = *reinterpret_cast<const float2 *>(S + (ra1 + 128 * k));
     }
-    if (h) {
-        w32_pretwiddle(a0);
-        w32_pretwiddle(a1);
-    }
-    fft_dif<16>(a0);
-    fft_dif<16>(a1);
-    __syncwarp();  // every lane has read both rows before the even half overwrites them
+    // The two rows run half a phase apart: each shared-memory round trip of one row (exchange store -> load -> use)
+    // is issued before, and lands under, an FFT of the other row; a0 / a1 are re-used as the landing registers.
     const int wa0 = exA + wr, wa1 = exB + wr, ea0 = exA + er, ea1 = exB + er;
+    if (h) w32_pretwiddle(a0);
+    fft_dif<16>(a0);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a0[i] = cmul(a0[i], twc[bitrev(i, 4)]);
+    __syncwarp();  // every lane has read both rows before the even half overwrites them
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         const int j2 = bitrev(i, 4);
-        *reinterpret_cast<float2 *>(S + ((wa0 ^ ((j2 & 7) << 4)) + 128 * j2)) = cmul(a0[i], twc[j2]);
-        *reinterpret_cast<float2 *>(S + ((wa1 ^ ((j2 & 7) << 4)) + 128 * j2)) = cmul(a1[i], twc[j2]);
+        *reinterpret_cast<float2 *>(S + ((wa0 ^ ((j2 & 7) << 4)) + 128 * j2)) = a0[i];
     }
     __syncwarp();
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
+    for (int i = 0; i < 8; ++i) {   // row A, second stage inputs: in flight during row B's first FFT
         const float4 v = *reinterpret_cast<const float4 *>(S + (ea0 ^ (i << 4)));
-        const float4 w = *reinterpret_cast<const float4 *>(S + (ea1 ^ (i << 4)));
         a0[2 * i] = make_float2(v.x, v.y);
         a0[2 * i + 1] = make_float2(v.z, v.w);
+    }
+    if (h) w32_pretwiddle(a1);
+    fft_dif<16>(a1);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const int j2 = bitrev(i, 4);
+        *reinterpret_cast<float2 *>(S + ((wa1 ^ ((j2 & 7) << 4)) + 128 * j2)) = cmul(a1[i], twc[j2]);
+    }
+    __syncwarp();  // exchange B complete; every lane's exchange reads of row A are done as well
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {   // row B, second stage inputs: in flight during row A's second FFT
+        const float4 w = *reinterpret_cast<const float4 *>(S + (ea1 ^ (i << 4)));
         a1[2 * i] = make_float2(w.x, w.y);
         a1[2 * i + 1] = make_float2(w.z, w.w);
     }
     fft_dif<16>(a0);
-    fft_dif<16>(a1);
-    __syncwarp();  // all exchange reads done before slots are written into the rows
     const uint32_t sw[8] = {sel0.x, sel0.y, sel0.z, sel0.w, sel1.x, sel1.y, sel1.z, sel1.w};
     unsigned char *rp0 = S + rowA, *rp1 = S + rowB;
 #pragma unroll
     for (int i = 0; i < 16; i += 2) {
         const uint32_t w = sw[i >> 1];
-        if (!(w & 0x8000u)) {
-            *reinterpret_cast<float2 *>(rp0 + (w & 0xFFFFu)) = a0[i];
-            *reinterpret_cast<float2 *>(rp1 + (w & 0xFFFFu)) = a1[i];
-        }
-        if ((int)w >= 0) {
-            *reinterpret_cast<float2 *>(rp0 + (w >> 16)) = a0[i + 1];
-            *reinterpret_cast<float2 *>(rp1 + (w >> 16)) = a1[i + 1];
-        }
+        if (!(w & 0x8000u)) *reinterpret_cast<float2 *>(rp0 + (w & 0xFFFFu)) = a0[i];
+        if ((int)w >= 0) *reinterpret_cast<float2 *>(rp0 + (w >> 16)) = a0[i + 1];
+    }
+    fft_dif<16>(a1);
+    __syncwarp();  // all exchange reads of row B done before its slots are written into the row
+#pragma unroll
+    for (int i = 0; i < 16; i += 2) {
+        const uint32_t w = sw[i >> 1];
+        if (!(w & 0x8000u)) *reinterpret_cast<float2 *>(rp1 + (w & 0xFFFFu)) = a1[i];
+        if ((int)w >= 0) *reinterpret_cast<float2 *>(rp1 + (w >> 16)) = a1[i + 1];
     }
 }
 
