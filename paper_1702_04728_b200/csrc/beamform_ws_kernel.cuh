@@ -330,6 +330,12 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
             const uint32_t ta = taddr0 + 128u * (uint32_t)st;
 #pragma unroll 1
             for (int half = 0; half < 2; ++half) {
+                // this lane's selected-bin slots: read now, so that the load lands during the copy and the barrier
+                const uint32_t xr = (uint32_t)(rx << 4) * 0x00010001u;
+                uint4 sel0 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16);
+                uint4 sel1 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16 + 8);
+                sel0 = make_uint4(sel0.x ^ xr, sel0.y ^ xr, sel0.z ^ xr, sel0.w ^ xr);
+                sel1 = make_uint4(sel1.x ^ xr, sel1.y ^ xr, sel1.z ^ xr, sel1.w ^ xr);
                 tile_from_tmem(S, kTileOfs, ta, rw, lane, half);
                 if (half == 1 && pp < 22) {   // stage drained: hand it back (the last two pairs have no successor)
                     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -337,11 +343,6 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
                 }
                 bar_sync(BAR_CONS, kCThreads);
                 {
-                    const uint32_t xr = (uint32_t)(rx << 4) * 0x00010001u;
-                    uint4 sel0 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16);
-                    uint4 sel1 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16 + 8);
-                    sel0 = make_uint4(sel0.x ^ xr, sel0.y ^ xr, sel0.z ^ xr, sel0.w ^ xr);
-                    sel1 = make_uint4(sel1.x ^ xr, sel1.y ^ xr, sel1.z ^ xr, sel1.w ^ xr);
 #pragma unroll 1
                     for (int rr = 0; rr < 4; rr += 2) {
                         const int rowA = row0 + rr * 8 * 2048, rowB = rowA + 8 * 2048;
