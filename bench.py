@@ -276,7 +276,7 @@ def run_cuda(args):
                      "frac": ach / fp32_peak, "traffic": traffic,
                      "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
                      "traffic_source": traffic_src, "algorithmic_bytes": in_bytes + out_bytes,
-                     "kernel": ("chime3::beamform_ws_kernel" if args.upchan == 128 and args.zero_pad in (256, 512)
+                     "kernel": ("chime3::beamform_ws_kernel" if args.upchan == 128
                                 else "chime::beamform_fused_kernel"), "kernel_ms": kern_ms,
                      "flops_per_chan_sample": fft_flops,
                      "note": f"FP32 peak = 148 SM x 128 lanes x 2 x {sm_mhz:.0f} MHz ({peak_kind} sm_max_mhz); "
