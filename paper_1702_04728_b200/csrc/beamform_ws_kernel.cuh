@@ -218,6 +218,9 @@ __device__ __forceinline__ void phase_c2(const unsigned char *S, const int col0,
     }
 }
 
+// P1 = true: zero_pad 256 (see the consumer set-up); a template parameter so that the default instantiation's
+// register allocation is untouched.
+template <bool P1>
 __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params prm) {
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *const S = smem;
@@ -305,7 +308,11 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
     } else {
         // ======================================= CONSUMERS =======================================
         asm volatile("setmaxnreg.inc.sync.aligned.u32 176;");
-        const int h = lane >> 4, l = lane & 15;
+        // P1 (zero_pad 256): only the even bins of the 512-point transform exist, so the two half-warps do not
+        // split the bin parities but the ROWS: lanes 0..15 take rows rw, rw + 16, lanes 16..31 rows rw + 8, rw + 24,
+        // every lane on the even-parity path (hp = 0) -- one phase-B call per residue instead of two.
+        const int hl = lane >> 4, l = lane & 15;
+        const int h = P1 ? 0 : hl;
         const int rx = rw & 7, xx = h ? 0 : rx;   // rows rw, rw + 8, rw + 16, rw + 24 share the swizzle
         const int rd = (((l >> 1) ^ rx) << 4) | ((l & 1) << 3);
         const int wr = (((l >> 1) ^ xx) << 4) | ((l & 1) << 3);
@@ -332,8 +339,8 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
             for (int half = 0; half < 2; ++half) {
                 // this lane's selected-bin slots: read now, so that the load lands during the copy and the barrier
                 const uint32_t xr = (uint32_t)(rx << 4) * 0x00010001u;
-                uint4 sel0 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16);
-                uint4 sel1 = *reinterpret_cast<const uint4 *>(s_sel + lane * 16 + 8);
+                uint4 sel0 = *reinterpret_cast<const uint4 *>(s_sel + (16 * h + l) * 16);
+                uint4 sel1 = *reinterpret_cast<const uint4 *>(s_sel + (16 * h + l) * 16 + 8);
                 sel0 = make_uint4(sel0.x ^ xr, sel0.y ^ xr, sel0.z ^ xr, sel0.w ^ xr);
                 sel1 = make_uint4(sel1.x ^ xr, sel1.y ^ xr, sel1.z ^ xr, sel1.w ^ xr);
                 tile_from_tmem(S, kTileOfs, ta, rw, lane, half);
@@ -343,10 +350,15 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
                 }
                 bar_sync(BAR_CONS, kCThreads);
                 {
+                    if constexpr (P1) {
+                        const int rowA = row0 + hl * 8 * 2048, rowB = rowA + 16 * 2048;
+                        phase_b_2rows(S, rowA, rowB, rowA, rowB, 0, rd, wr, er, sel0, sel1, twc);
+                    } else {
 #pragma unroll 1
-                    for (int rr = 0; rr < 4; rr += 2) {
-                        const int rowA = row0 + rr * 8 * 2048, rowB = rowA + 8 * 2048;
-                        phase_b_2rows(S, rowA, rowB, h ? exw : rowA, h ? exw + 2048 : rowB, h, rd, wr, er, sel0, sel1, twc);
+                        for (int rr = 0; rr < 4; rr += 2) {
+                            const int rowA = row0 + rr * 8 * 2048, rowB = rowA + 8 * 2048;
+                            phase_b_2rows(S, rowA, rowB, h ? exw : rowA, h ? exw + 2048 : rowB, h, rd, wr, er, sel0, sel1, twc);
+                        }
                     }
                 }
                 bar_sync(BAR_CONS, kCThreads);

@@ -251,7 +251,9 @@ bool build_tables(chime_bf_plan *pl) {
         CUDA_TRY(cudaMemcpyToSymbol(chime2::c_tw128, tw128.data(), sizeof(float2) * 128));
         CUDA_TRY(cudaFuncSetAttribute(chime2::beamform_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       chime2::kSmemBytes));
-        CUDA_TRY(cudaFuncSetAttribute(chime3::beamform_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        CUDA_TRY(cudaFuncSetAttribute(chime3::beamform_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      chime3::kSmemBytesWs));
+        CUDA_TRY(cudaFuncSetAttribute(chime3::beamform_ws_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       chime3::kSmemBytesWs));
     }
     CUDA_TRY(cudaMalloc((void **)&pl->d_delay, (size_t)pl->C * 16 * sizeof(int32_t)));
@@ -345,8 +347,10 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
             mp.bfrag = pl->d_bfrag + (size_t)pass * pl->C * 2 * 2 * 256 * 16;
             mp.slot = pl->d_slot + (size_t)pass * pl->C * 512;
             mp.slot_of_m = pl->d_slot_of_m + (size_t)pass * pl->C * 256;
-            if (pl->use_ws)
-                chime3::beamform_ws_kernel<<<n_chan * n_fr * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
+            if (pl->use_ws && pl->NP == 256)
+                chime3::beamform_ws_kernel<true><<<n_chan * n_fr * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
+            else if (pl->use_ws)
+                chime3::beamform_ws_kernel<false><<<n_chan * n_fr * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
             else
                 chime2::beamform_mma_kernel<<<n_chan * n_fr * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
         }
