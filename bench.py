@@ -276,7 +276,8 @@ def run_cuda(args):
                      "frac": ach / fp32_peak, "traffic": traffic,
                      "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
                      "traffic_source": traffic_src, "algorithmic_bytes": in_bytes + out_bytes,
-                     "kernel": ("chime3::beamform_ws_kernel" if args.upchan == 128
+                     "kernel": (("chime3::beamform_ws_kernel<true>" if args.zero_pad == 256 else
+                                 "chime3::beamform_ws_kernel<false>") if args.upchan == 128
                                 else "chime::beamform_fused_kernel"), "kernel_ms": kern_ms,
                      "flops_per_chan_sample": fft_flops,
                      "note": f"FP32 peak = 148 SM x 128 lanes x 2 x {sm_mhz:.0f} MHz ({peak_kind} sm_max_mhz); "
@@ -288,7 +289,7 @@ def run_cuda(args):
         "gpu_launches": args.steps * plan.launches_per_execute,
         "clocks": clocks,
     }
-    if not args.no_cpu_baseline and world >= 1:
+    if not args.no_cpu_baseline and world == 1:     # the oracle is timed on rank 0 at N = 1 only
         dt, cs, cores = oracle_sample(256)
         v = cs * BYTES_PER_CHAN_SAMPLE / dt / 1e9
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
