@@ -176,3 +176,20 @@ def test_all_kernel_generations_agree_with_oracle(bf, orc, kernel, monkeypatch):
                                 cells, 512, 128)
     print(f"{kernel}: worst rel err {worst:.2e}, u8 diff frac {frac:.2e}")
     plan.destroy()
+
+
+@pytest.mark.parametrize("NP,U", [(512, 128), (256, 128), (1024, 128), (512, 256)])
+def test_repeated_executes_are_bit_identical(bf, NP, U):
+    """The kernels hand tiles between warps through shared and tensor memory behind named barriers; a missing
+    barrier would show as run-to-run differences.  30 executes of the same input (6 channels x 10 frames, so that
+    several CTAs share every SM and the waves overlap) must give identical bytes and identical floats."""
+    C, T = 6, 10 * 3 * U
+    plan = bf.plan_create_ex(C, zero_pad=NP, upchan_len=U, n_time=T, gains=synth.gains(3, C))
+    d_in = synth.noise_bytes(77, C, T, device="cuda")
+    ref_u8 = plan.execute(d_in).clone()
+    ref_f32 = plan.execute_f32(d_in).clone()
+    for _ in range(30):
+        assert torch.equal(plan.execute(d_in), ref_u8)
+    for _ in range(5):
+        assert torch.equal(plan.execute_f32(d_in), ref_f32)
+    plan.destroy()
