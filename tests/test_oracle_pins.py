@@ -339,3 +339,39 @@ def test_quantize_rne_and_saturation(orc):
     I = np.array([0.0, 32.0, 96.0, 160.0, 64.0 * 127.0, 1e9, -1e9, 64.0 * 0.49, 64 * 0.51])
     q = orc.quantize(I, 1.0 / 64.0, 128.0)
     assert list(q) == [128, 128, 130, 130, 255, 255, 0, 128, 129]   # 128.5->128, 129.5->130, 130.5->130
+
+
+def test_p14_frequency_summed_beam_width_sec31(orc):
+    """P14 -- PAPER.md:80: the frequency-summed formed beam is ~0.5 deg wide (FWHM) at zenith and ~2.8 deg at 10 deg
+    elevation.  Oracle N-S beamformer (direct sums, nearest-bin clamping at every frequency) on plane waves swept in
+    angle, summed over 64 frequencies of the band; see tests/golden/beam_fwhm_sec31.json for the reading."""
+    import json
+    import os
+    gold = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "beam_fwhm_sec31.json")))
+    d, c0 = 0.3048, 299792458.0
+    freqs = 800.0 - 0.390625 * np.arange(0, 1024, 16)
+    n = np.arange(256)
+
+    def widths(s0, span_deg, npts=321):
+        th = np.arcsin(s0) + np.deg2rad(np.linspace(-span_deg, span_deg, npts))
+        power = np.zeros(npts)
+        for f in freqs:
+            J = orc.ns_index_sintheta(f, [s0], 512)
+            x = np.exp(2j * np.pi * f * 1e6 * d * np.outer(np.sin(th), n) / c0).reshape(npts, 1, 1, 256)
+            w = np.zeros((1, 1, 2))
+            w[0, 0, 0] = 1.0
+            Z = orc.beamform(x, np.ones((1, 1, 256), dtype=complex), J, w, 512)
+            power += np.abs(Z[:, 0, 0, 0]) ** 2
+        out = []
+        for patt in (power / power.max(), np.sqrt(power / power.max())):     # power and voltage pattern
+            above = np.where(patt >= 0.5)[0]
+            out.append(float(np.rad2deg(th[above[-1]] - th[above[0]])))
+        return out
+
+    p_zen, v_zen = widths(0.0, 1.0)
+    p_low, v_low = widths(np.sin(np.deg2rad(80.0)), 8.0)
+    ratio = gold["fwhm_10deg_elevation_deg"] / gold["fwhm_zenith_deg"]
+    assert abs(p_low / p_zen - ratio) < 0.15 * ratio and abs(v_low / v_zen - ratio) < 0.15 * ratio
+    assert abs(v_zen - gold["fwhm_zenith_deg"]) < 0.2 * gold["fwhm_zenith_deg"]
+    assert abs(v_low - gold["fwhm_10deg_elevation_deg"]) < 0.2 * gold["fwhm_10deg_elevation_deg"]
+    assert 0.28 < p_zen < 0.36          # 0.886 lambda / D at the band's power-weighted mean wavelength
