@@ -33,10 +33,10 @@ enum { BAR_FULL0 = 1, BAR_FULL1 = 2, BAR_EMPTY0 = 3, BAR_EMPTY1 = 4, BAR_CONS = 
 __device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" :: "r"(id), "r"(n) : "memory"); }
 
-// ---- producer: phase A for residues RHO and RHO + 4, feeds 32 pw .. 32 pw + 31, into TMEM ----------------
+// ---- producer: phase A for residues RHO and RHO + 4, feeds 32 pw + 8 hh .. + 7, into TMEM ----------------
 template <int RHO>
-__device__ __forceinline__ void produce_pair(const unsigned char *raw, const uint2 *bfrag_cpe, const int pw,
-                                             const int lane, const uint32_t taddr) {
+__device__ __forceinline__ void produce_chunk(const unsigned char *raw, const uint2 *bfrag_cpe, const int pw,
+                                              const int lane, const uint32_t taddr, const int hh) {
     constexpr bool ODD = (RHO & 1) != 0;
     const int g = lane >> 2, tq = lane & 3;
     const __half2 nbE = __floats2half2_rn(-32.0f / 512.0f, -32.0f / 512.0f);
@@ -47,8 +47,7 @@ __device__ __forceinline__ void produce_pair(const unsigned char *raw, const uin
     const float ss = (tq < 2 ? 1.0f : -1.0f) * (ODD ? 0.70710678118654752440f : 1.0f);
     const uint2 *bf_l = bfrag_cpe + (size_t)(32 * pw) * 16 + (lane & 15);
 
-#pragma unroll 1
-    for (int hh = 0; hh < 4; ++hh) {        // 8 feeds at a time
+    {                                        // 8 feeds at a time
         uint32_t aE[2][8], aO[2][8];
         const unsigned char *raw_h = raw_t + (((4 * pw + hh) ^ pz) << 3);
 #pragma unroll
@@ -98,6 +97,14 @@ __device__ __forceinline__ void produce_pair(const unsigned char *raw, const uin
             tmem_st8(taddr + 32 * hh + 4 * i, z[0][0], z[0][1], z[1][0], z[1][1], z[0][2], z[0][3], z[1][2], z[1][3]);
         }
     }
+}
+
+// all 32 feeds of producer warp pw (four chunks)
+template <int RHO>
+__device__ __forceinline__ void produce_pair(const unsigned char *raw, const uint2 *bfrag_cpe, const int pw,
+                                             const int lane, const uint32_t taddr) {
+#pragma unroll 1
+    for (int hh = 0; hh < 4; ++hh) produce_chunk<RHO>(raw, bfrag_cpe, pw, lane, taddr, hh);
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
