@@ -143,6 +143,33 @@ int chime_bf_dedisp_delays(const chime_bf_plan *plan, double dm, double f_ref_mh
 int chime_bf_dedisperse(chime_bf_plan *plan, void *cuda_stream, const uint8_t *beams_u8, double dm,
                         double f_ref_mhz, uint32_t *out_u32, int n_out);
 
+/*
+ * Beam-major exchange fused into the beamformer (the formed beams leave the X-engine
+ * node "to a FRB backend" per beam): with the coarse channels sharded over W GPUs (one plan per GPU, no collective
+ * inside the beamformer), the consumer of the beams wants all channels of a SUBSET of beams.  This call runs the
+ * same pass as chime_bf_execute but its epilogue stores each beam's 16 bytes straight into the receive buffer of
+ * the rank that owns the beam: beam b = ew*256 + ns of (global channel cg, frame r) goes to rank d = b / (1024/W),
+ * at peer_out[d][cg][r][b - d*1024/W][16].  With peer-mapped pointers (CUDA IPC / symmetric memory over NVLink) the
+ * all-to-all IS the kernel's store; with W = 1 or local pointers it is a plain re-layout.  No NCCL call, no staging.
+ *   peer_out      HOST array of n_peers DEVICE pointers (copied to a plan-owned device table on `cuda_stream`);
+ *                 buffer d has shape [C_total][n_frames][1024/n_peers][16], 16-byte aligned, caller-owned.
+ *   n_peers       W; must divide 1024, <= 64
+ *   chan_global0  global index of this plan's channel 0 (channels chan_global0 .. + n_coarse - 1 are written)
+ * The caller synchronises the ranks (all writers done) before any rank reads its receive buffer.
+ */
+int chime_bf_execute_beam_major(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8,
+                                uint8_t *const *peer_out, int n_peers, int chan_global0);
+
+/* chime_bf_dedisperse on a beam subset, e.g. a rank's receive buffer after the beam-major exchange: DEVICE beams_u8
+ * [n_coarse][n_frames][n_beams][16], n_beams a multiple of 32; HOST freq_mhz[n_coarse]; DEVICE delay_scratch
+ * [n_coarse*16] int32 (caller-owned); DEVICE out_u32 [n_beams][n_out], n_out = n_frames - max delay.  Same formula,
+ * same kernel as chime_bf_dedisperse; needs no plan. */
+int chime_bf_dedisp_delays_ex(const double *freq_mhz, int n_coarse, int upchan_len, double dm, double f_ref_mhz,
+                              int32_t *host_out /* [n_coarse][16] or NULL */, int *max_delay /* HOST, or NULL */);
+int chime_bf_dedisperse_beams(void *cuda_stream, const uint8_t *beams_u8, int n_coarse, const double *freq_mhz,
+                              int n_frames, int n_beams, int upchan_len, double dm, double f_ref_mhz,
+                              int32_t *delay_scratch, uint32_t *out_u32, int n_out);
+
 /* Copy of the clamped N-S bin index table J (eq. (1),(2)): HOST out, [C][256] int32. */
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out);
 

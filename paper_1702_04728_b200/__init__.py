@@ -19,7 +19,8 @@ EXPORTS = [
     "chime_bf_execute_host", "chime_bf_get_ns_index", "chime_bf_debug_unpack", "chime_bf_n_frames",
     "chime_bf_in_bytes", "chime_bf_out_elems", "chime_bf_launches_per_execute", "chime_bf_destroy",
     "chime_bf_last_error", "chime_bf_update_gains", "chime_bf_update_ew_angles", "chime_bf_update_pointings",
-    "chime_bf_dedisp_delays", "chime_bf_dedisperse",
+    "chime_bf_dedisp_delays", "chime_bf_dedisperse", "chime_bf_execute_beam_major", "chime_bf_dedisperse_beams",
+    "chime_bf_dedisp_delays_ex",
 ]
 
 
@@ -78,6 +79,12 @@ def load_library():
     lib.chime_bf_dedisp_delays.argtypes = [vp, ctypes.c_double, ctypes.c_double, vp, ctypes.POINTER(ci)]
     lib.chime_bf_dedisperse.restype = ci
     lib.chime_bf_dedisperse.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp, ci]
+    lib.chime_bf_execute_beam_major.restype = ci
+    lib.chime_bf_execute_beam_major.argtypes = [vp, vp, vp, vp, ci, ci]
+    lib.chime_bf_dedisp_delays_ex.restype = ci
+    lib.chime_bf_dedisp_delays_ex.argtypes = [vp, ci, ci, ctypes.c_double, ctypes.c_double, vp, ctypes.POINTER(ci)]
+    lib.chime_bf_dedisperse_beams.restype = ci
+    lib.chime_bf_dedisperse_beams.argtypes = [vp, vp, ci, vp, ci, ci, ci, ctypes.c_double, ctypes.c_double, vp, vp, ci]
     lib.chime_bf_n_frames.restype = ci
     lib.chime_bf_n_frames.argtypes = [vp]
     lib.chime_bf_in_bytes.restype = ctypes.c_size_t
@@ -190,6 +197,15 @@ class Plan:
         self._check(load_library().chime_bf_update_pointings(self._h, _stream_ptr(stream), float(f_ref_mhz),
                                                              None if s is None else s.ctypes.data))
 
+    def execute_beam_major(self, in_u8, peer_ptrs, chan_global0, stream=None):
+        """chime_bf_execute_beam_major: peer_ptrs = the W receive buffers (CUDA uint8 tensors of shape
+        [C_total][n_frames][1024/W][16], or raw device pointers of peer-mapped buffers)."""
+        self._check_in(in_u8)
+        ptrs = [p if isinstance(p, int) else p.data_ptr() for p in peer_ptrs]
+        arr = (ctypes.c_void_p * len(ptrs))(*ptrs)
+        self._check(load_library().chime_bf_execute_beam_major(self._h, _stream_ptr(stream), in_u8.data_ptr(), arr,
+                                                               len(ptrs), int(chan_global0)))
+
     def dedisp_delays(self, dm, f_ref_mhz=0.0):
         """chime_bf_dedisp_delays -> (delay [n_coarse][16] int32, n_out)."""
         tab = np.zeros((self.n_coarse, N_FINE), dtype=np.int32)
@@ -236,6 +252,34 @@ class Plan:
             self.destroy()
         except Exception:
             pass
+
+
+def dedisperse_beams(beams_u8, freq_mhz, dm, upchan_len=128, f_ref_mhz=0.0, stream=None):
+    """chime_bf_dedisperse_beams: uint8 beams [C][R][n_beams][16] (any beam subset) -> int32 [n_beams][n_out].
+    n_out = R - max delay comes from chime_bf_dedisp_delays_ex."""
+    import torch
+    assert beams_u8.is_cuda and beams_u8.dtype == torch.uint8 and beams_u8.is_contiguous() and beams_u8.dim() == 4
+    C, R, nb, nf = beams_u8.shape
+    assert nf == N_FINE
+    f = np.ascontiguousarray(freq_mhz, dtype=np.float64)
+    if f.size != C:
+        raise ValueError("freq_mhz must have one entry per coarse channel")
+    mx = ctypes.c_int(0)
+    rc = load_library().chime_bf_dedisp_delays_ex(f.ctypes.data, C, upchan_len, float(dm), float(f_ref_mhz), None,
+                                                  ctypes.byref(mx))
+    if rc != 0:
+        raise ChimeBfError(f"chime_bf error {rc}: {last_error()}")
+    n_out = R - mx.value
+    if n_out < 1:
+        raise ChimeBfError(f"dedisperse_beams: the DM {dm} sweep is longer than the {R}-frame buffer")
+    out = torch.empty((nb, n_out), dtype=torch.int32, device=beams_u8.device)
+    scratch = torch.empty(C * 16, dtype=torch.int32, device=beams_u8.device)
+    rc = load_library().chime_bf_dedisperse_beams(_stream_ptr(stream), beams_u8.data_ptr(), C, f.ctypes.data, R, nb,
+                                                  upchan_len, float(dm), float(f_ref_mhz), scratch.data_ptr(),
+                                                  out.data_ptr(), n_out)
+    if rc != 0:
+        raise ChimeBfError(f"chime_bf error {rc}: {last_error()}")
+    return out
 
 
 def plan_create(n_coarse, gains=None, ew_angles=EW_ANGLES_DEG, zero_pad=512, upchan_len=128):

@@ -45,10 +45,24 @@ struct KernelParams {
     int n_frames;            // R
     int chan0;               // first channel this launch processes (grid covers n_chan channels from here)
     int frame0, n_frames_launch;   // frame range of this launch within each channel
+    // beam-major exchange (chime_bf_execute_beam_major): peer_out[d] = receive buffer of rank d,
+    // [C_total][R][1024 / n_peers][16]; this launch's channel c is global channel chan_global0 + c.  nullptr = off.
+    uint8_t *const *peer_out;
+    int n_peers, chan_global0;
     float norm;              // 1/(N N_c U)
     float qscale;            // norm * scale
     float qoffset;
 };
+
+// Beam-major exchange addressing: beam b = ew * 256 + ns of (global channel cg, frame Rf) goes to rank
+// d = b / (1024 / n_peers), at [cg][Rf][b - d * 1024 / n_peers][16 fine] of that rank's receive buffer: the
+// all-to-all corner turn (channel-sharded -> beam-sharded) is the epilogue's 16-byte store itself; with peer-mapped
+// pointers the store crosses NVLink.
+__device__ __forceinline__ uint4 *beam_major_dst(uint8_t *const *peer_out, const int n_peers, const int cg,
+                                                 const int n_frames, const int Rf, const int b) {
+    const int bpr = 1024 / n_peers, d = b / bpr;
+    return reinterpret_cast<uint4 *>(peer_out[d] + (((size_t)cg * n_frames + Rf) * bpr + (b - d * bpr)) * 16);
+}
 
 template <int P>
 __host__ __device__ constexpr int exch_bufs_per_warp() { return P <= 2 ? 2 : P; }
@@ -320,7 +334,11 @@ beamform_fused_kernel(const KernelParams prm) {
         qb[tid] = make_uint4(q[0], q[1], q[2], q[3]);
         __syncthreads();
         const int s = s_slot_of_m[tid];
-        reinterpret_cast<uint4 *>(prm.out_u8 + out_base)[tid] = qb[s];
+        if (prm.peer_out != nullptr) {
+            *beam_major_dst(prm.peer_out, prm.n_peers, prm.chan_global0 + c, prm.n_frames, Rf, e * 256 + tid) = qb[s];
+        } else {
+            reinterpret_cast<uint4 *>(prm.out_u8 + out_base)[tid] = qb[s];
+        }
     }
 }
 

@@ -54,6 +54,8 @@ struct Params {
     int n_frames;
     int chan0;                // first channel this launch processes
     int frame0, n_frames_launch;   // frame range of this launch within each channel
+    uint8_t *const *peer_out;      // beam-major exchange (see chime::beam_major_dst), nullptr = off
+    int n_peers, chan_global0;
     float norm, qscale, qoffset;
 };
 

@@ -418,7 +418,12 @@ __global__ void __launch_bounds__(kThreads, 1) beamform_ws_kernel(const Params p
                 qb[sl] = make_uint4(q[0], q[1], q[2], q[3]);
                 bar_sync(BAR_CONS, kCThreads);
                 const int s = s_slot_of_m[sl];
-                if (s >= 0) reinterpret_cast<uint4 *>(prm.out_u8 + out_base)[sl] = qb[s];
+                if (s >= 0) {
+                    if (prm.peer_out != nullptr)
+                        *chime::beam_major_dst(prm.peer_out, prm.n_peers, prm.chan_global0 + c, prm.n_frames, Rf, e * 256 + sl) = qb[s];
+                    else
+                        reinterpret_cast<uint4 *>(prm.out_u8 + out_base)[sl] = qb[s];
+                }
             }
             bar_sync(BAR_CONS, kCThreads);
         }

@@ -60,6 +60,7 @@ struct chime_bf_plan {
     std::vector<cudaEvent_t> copy_done;   // one event per channel
     cudaEvent_t entry = nullptr;
     int host_parts = 1;                   // execute_host: frame ranges per channel
+    uint8_t **d_peer_out = nullptr;       // execute_beam_major: device copy of the peers' receive-buffer pointers (<= 64)
     int32_t *d_delay = nullptr;   // [C][16] dedispersion delays of the last chime_bf_dedisperse call
 };
 
@@ -257,23 +258,24 @@ bool build_tables(chime_bf_plan *pl) {
                                       chime3::kSmemBytesWs));
     }
     CUDA_TRY(cudaMalloc((void **)&pl->d_delay, (size_t)pl->C * 16 * sizeof(int32_t)));
+    CUDA_TRY(cudaMalloc((void **)&pl->d_peer_out, 64 * sizeof(uint8_t *)));
     return upload(&pl->d_tw_np, tw_np) && upload(&pl->d_tw_u, tw_u);
 }
 
 // Dispersion delay of fine channel (c, g) relative to f_ref, in output frames (reading F1):
 //   f = f_c + (g - 7.5) * 0.390625/16 MHz,  x = K_DM * DM * (f^-2 - f_ref^-2) / (3 U * 2.56 us),
 //   delay = floor(x + 0.5),  K_DM = 4148.808 s MHz^2 cm^3 / pc.   Returns the largest delay.
-int dedisp_table(const chime_bf_plan *pl, double dm, double fref_mhz, std::vector<int32_t> &tab) {
-    const double fine = 0.390625 / 16.0, tau = 3.0 * (double)pl->U * 2.56e-6;
+int dedisp_table(const double *freq, int C, int U, double dm, double fref_mhz, std::vector<int32_t> &tab) {
+    const double fine = 0.390625 / 16.0, tau = 3.0 * (double)U * 2.56e-6;
     if (!(fref_mhz > 0)) {
         fref_mhz = 0;
-        for (int c = 0; c < pl->C; ++c) fref_mhz = std::max(fref_mhz, pl->freq[c] + 7.5 * fine);
+        for (int c = 0; c < C; ++c) fref_mhz = std::max(fref_mhz, freq[c] + 7.5 * fine);
     }
-    tab.resize((size_t)pl->C * 16);
+    tab.resize((size_t)C * 16);
     int mx = 0;
-    for (int c = 0; c < pl->C; ++c)
+    for (int c = 0; c < C; ++c)
         for (int g = 0; g < 16; ++g) {
-            const double f = pl->freq[c] + ((double)g - 7.5) * fine;
+            const double f = freq[c] + ((double)g - 7.5) * fine;
             const double x = 4148.808 * dm * (1.0 / (f * f) - 1.0 / (fref_mhz * fref_mhz)) / tau;
             const int d = (int)std::floor(x + 0.5);
             tab[(size_t)c * 16 + g] = d;
@@ -297,10 +299,11 @@ cudaError_t launch(const chime::KernelParams &kp, int n_cta, cudaStream_t st) {
 }
 
 int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, float *out_f32, int chan0 = 0,
-        int n_chan = -1, int frame0 = 0, int n_fr = -1) {
+        int n_chan = -1, int frame0 = 0, int n_fr = -1, uint8_t *const *peer_out = nullptr, int n_peers = 0,
+        int chan_global0 = 0) {
     if (pl && n_chan < 0) n_chan = pl->C;
     if (pl && n_fr < 0) n_fr = pl->R;
-    if (!pl || !in || (!out_u8 && !out_f32)) {
+    if (!pl || !in || (!out_u8 && !out_f32 && !peer_out)) {
         set_err("execute: null argument");
         return CHIME_BF_E_INVALID_ARG;
     }
@@ -322,6 +325,9 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
     kp.chan0 = chan0;
     kp.frame0 = frame0;
     kp.n_frames_launch = n_fr;
+    kp.peer_out = peer_out;
+    kp.n_peers = n_peers;
+    kp.chan_global0 = chan_global0;
     kp.norm = pl->norm;
     kp.qscale = pl->norm * pl->scale;
     kp.qoffset = pl->offset;
@@ -340,6 +346,9 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         mp.chan0 = chan0;
         mp.frame0 = frame0;
         mp.n_frames_launch = n_fr;
+        mp.peer_out = peer_out;
+        mp.n_peers = n_peers;
+        mp.chan_global0 = chan_global0;
         mp.norm = pl->norm;
         mp.qscale = pl->norm * pl->scale;
         mp.qoffset = pl->offset;
@@ -374,6 +383,35 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         set_err("kernel launch failed: %s", cudaGetErrorString(e));
         return CHIME_BF_E_CUDA;
     }
+    return CHIME_BF_OK;
+}
+
+int launch_dedisperse(void *stream, const uint8_t *beams_u8, int C, int R, int n_beams, const std::vector<int32_t> &tab,
+                      int32_t *d_delay, uint32_t *out_u32, int n_out) {
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(d_delay, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        chime_dd::Params dp;
+        dp.in = reinterpret_cast<const uint32_t *>(beams_u8);
+        dp.delay = d_delay;
+        dp.out = out_u32;
+        dp.C = C;
+        dp.R = R;
+        dp.n_out = n_out;
+        dp.n_beams = n_beams;
+        const int bt = n_beams / chime_dd::kBeamsPerCta, tt = (n_out + chime_dd::kTR - 1) / chime_dd::kTR;
+        // fill 148 SMs x 16 resident CTAs: split the channel loop when beams x time tiles are too few
+        int n_split = std::min(C, std::max(1, (148 * 16 + bt * tt - 1) / (bt * tt)));
+        dp.c_per_split = (C + n_split - 1) / n_split;
+        n_split = (C + dp.c_per_split - 1) / dp.c_per_split;
+        if (n_split > 1) e = cudaMemsetAsync(out_u32, 0, (size_t)n_beams * n_out * sizeof(uint32_t), st);
+        if (e == cudaSuccess) {
+            dim3 grid(bt, tt, n_split);
+            chime_dd::dedisperse_kernel<<<grid, chime_dd::kThreads, 0, st>>>(dp);
+            e = cudaGetLastError();
+        }
+    }
+    if (e != cudaSuccess) { set_err("dedisperse: %s", cudaGetErrorString(e)); return CHIME_BF_E_CUDA; }
     return CHIME_BF_OK;
 }
 
@@ -465,6 +503,28 @@ int chime_bf_execute(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, ui
 
 int chime_bf_execute_f32(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, float *out_f32) {
     return run(plan, stream, in_u8, nullptr, out_f32);
+}
+
+int chime_bf_execute_beam_major(chime_bf_plan *pl, void *stream, const uint8_t *in_u8, uint8_t *const *peer_out,
+                                int n_peers, int chan_global0) {
+    if (!pl || !in_u8 || !peer_out) { set_err("execute_beam_major: null argument"); return CHIME_BF_E_INVALID_ARG; }
+    if (n_peers < 1 || n_peers > 64 || (1024 % n_peers) != 0 || chan_global0 < 0) {
+        set_err("execute_beam_major: n_peers must divide 1024 and be <= 64 (got %d), chan_global0 >= 0", n_peers);
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    for (int d = 0; d < n_peers; ++d)
+        if (!peer_out[d] || ((uintptr_t)peer_out[d] & 15)) {
+            set_err("execute_beam_major: peer buffer %d is null or not 16-byte aligned", d);
+            return CHIME_BF_E_ALIGNMENT;
+        }
+    if (pl->use_mma && !pl->use_ws) {
+        set_err("execute_beam_major: not available with CHIME_BF_KERNEL=v2");
+        return CHIME_BF_E_UNSUPPORTED;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(pl->d_peer_out, peer_out, n_peers * sizeof(uint8_t *), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { set_err("execute_beam_major: %s", cudaGetErrorString(e)); return CHIME_BF_E_CUDA; }
+    return run(pl, stream, in_u8, nullptr, nullptr, 0, -1, 0, -1, pl->d_peer_out, n_peers, chan_global0);
 }
 
 int chime_bf_execute_host(chime_bf_plan *pl, void *stream, const uint8_t *in_host, uint8_t *out_host) {
@@ -571,7 +631,7 @@ int chime_bf_update_pointings(chime_bf_plan *pl, void *stream, double f_ref_mhz,
 int chime_bf_dedisp_delays(const chime_bf_plan *pl, double dm, double f_ref_mhz, int32_t *host_out, int *n_out) {
     if (!pl || !(dm >= 0)) { set_err("dedisp_delays: bad argument"); return CHIME_BF_E_INVALID_ARG; }
     std::vector<int32_t> tab;
-    const int mx = dedisp_table(pl, dm, f_ref_mhz, tab);
+    const int mx = dedisp_table(pl->freq.data(), pl->C, pl->U, dm, f_ref_mhz, tab);
     for (int32_t d : tab)
         if (d < 0) { set_err("dedisp_delays: f_ref below a fine channel (negative delay)"); return CHIME_BF_E_INVALID_ARG; }
     if (host_out) memcpy(host_out, tab.data(), tab.size() * sizeof(int32_t));
@@ -591,30 +651,45 @@ int chime_bf_dedisperse(chime_bf_plan *pl, void *stream, const uint8_t *beams_u8
         set_err("dedisperse: n_out must be n_frames - max delay = %d (got %d)", n_full, n_out);
         return CHIME_BF_E_INVALID_ARG;
     }
-    cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = cudaMemcpyAsync(pl->d_delay, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) {
-        chime_dd::Params dp;
-        dp.in = reinterpret_cast<const uint32_t *>(beams_u8);
-        dp.delay = pl->d_delay;
-        dp.out = out_u32;
-        dp.C = pl->C;
-        dp.R = pl->R;
-        dp.n_out = n_out;
-        const int bt = 1024 / chime_dd::kBeamsPerCta, tt = (n_out + chime_dd::kTR - 1) / chime_dd::kTR;
-        // fill 148 SMs x 16 resident CTAs: split the channel loop when beams x time tiles are too few
-        int n_split = std::min(pl->C, std::max(1, (148 * 16 + bt * tt - 1) / (bt * tt)));
-        dp.c_per_split = (pl->C + n_split - 1) / n_split;
-        n_split = (pl->C + dp.c_per_split - 1) / dp.c_per_split;
-        if (n_split > 1) e = cudaMemsetAsync(out_u32, 0, (size_t)1024 * n_out * sizeof(uint32_t), st);
-        if (e == cudaSuccess) {
-            dim3 grid(bt, tt, n_split);
-            chime_dd::dedisperse_kernel<<<grid, chime_dd::kThreads, 0, st>>>(dp);
-            e = cudaGetLastError();
-        }
+    return launch_dedisperse(stream, beams_u8, pl->C, pl->R, 1024, tab, pl->d_delay, out_u32, n_out);
+}
+
+int chime_bf_dedisp_delays_ex(const double *freq_mhz, int n_coarse, int upchan_len, double dm, double f_ref_mhz,
+                              int32_t *host_out, int *max_delay) {
+    if (!freq_mhz || n_coarse < 1 || !(dm >= 0) || (upchan_len != 128 && upchan_len != 256)) {
+        set_err("dedisp_delays_ex: bad argument");
+        return CHIME_BF_E_INVALID_ARG;
     }
-    if (e != cudaSuccess) { set_err("dedisperse: %s", cudaGetErrorString(e)); return CHIME_BF_E_CUDA; }
+    std::vector<int32_t> tab;
+    const int mx = dedisp_table(freq_mhz, n_coarse, upchan_len, dm, f_ref_mhz, tab);
+    for (int32_t d : tab)
+        if (d < 0) { set_err("dedisp_delays_ex: f_ref below a fine channel (negative delay)"); return CHIME_BF_E_INVALID_ARG; }
+    if (host_out) memcpy(host_out, tab.data(), tab.size() * sizeof(int32_t));
+    if (max_delay) *max_delay = mx;
     return CHIME_BF_OK;
+}
+
+int chime_bf_dedisperse_beams(void *stream, const uint8_t *beams_u8, int n_coarse, const double *freq_mhz, int n_frames,
+                              int n_beams, int upchan_len, double dm, double f_ref_mhz, int32_t *delay_scratch,
+                              uint32_t *out_u32, int n_out) {
+    if (!beams_u8 || !freq_mhz || !delay_scratch || !out_u32 || n_coarse < 1 || n_frames < 1 || !(dm >= 0)) {
+        set_err("dedisperse_beams: bad argument");
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    if (n_beams < 32 || n_beams % 32 || (upchan_len != 128 && upchan_len != 256)) {
+        set_err("dedisperse_beams: n_beams must be a positive multiple of 32, upchan_len 128 or 256");
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    if ((uintptr_t)beams_u8 & 15) { set_err("dedisperse_beams: input must be 16-byte aligned"); return CHIME_BF_E_ALIGNMENT; }
+    std::vector<int32_t> tab;
+    const int mx = dedisp_table(freq_mhz, n_coarse, upchan_len, dm, f_ref_mhz, tab);
+    for (int32_t d : tab)
+        if (d < 0) { set_err("dedisperse_beams: f_ref below a fine channel (negative delay)"); return CHIME_BF_E_INVALID_ARG; }
+    if (n_frames - mx < 1 || n_out != n_frames - mx) {
+        set_err("dedisperse_beams: n_out must be n_frames - max delay = %d (got %d)", n_frames - mx, n_out);
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    return launch_dedisperse(stream, beams_u8, n_coarse, n_frames, n_beams, tab, delay_scratch, out_u32, n_out);
 }
 
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out) {
@@ -664,6 +739,7 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_stage_in);
     cudaFree(pl->d_stage_out);
     cudaFree(pl->d_delay);
+    cudaFree(pl->d_peer_out);
     for (cudaEvent_t ev : pl->copy_done)
         if (ev) cudaEventDestroy(ev);
     if (pl->entry) cudaEventDestroy(pl->entry);

@@ -22,10 +22,11 @@ constexpr int kBeamsPerCta = 32; // 128 threads = 32 beams x 4 quads
 constexpr int kThreads = 128;
 
 struct Params {
-    const uint32_t *in;      // [C][R][1024][4] words (4 fine channels per word, little endian)
+    const uint32_t *in;      // [C][R][n_beams][4] words (4 fine channels per word, little endian)
     const int32_t *delay;    // [C][16]
-    uint32_t *out;           // [1024][n_out]
+    uint32_t *out;           // [n_beams][n_out]
     int C, R, n_out;
+    int n_beams;             // beams in the array (1024, or 1024 / W after the beam-major exchange); multiple of 32
     int c_per_split;         // channels per blockIdx.z slice; > 1 slice: out is pre-zeroed and summed with atomicAdd (exact)
 };
 
@@ -38,7 +39,7 @@ __global__ void __launch_bounds__(kThreads, 4) dedisperse_kernel(const Params p)
 #pragma unroll
     for (int r = 0; r < kTR; ++r) acc[r] = 0u;
     const int n_valid = min(kTR, p.n_out - r0);      // ragged last tile
-    const size_t frame_words = 1024 * 4;
+    const size_t frame_words = (size_t)p.n_beams * 4;
     const int c_lo = blockIdx.z * p.c_per_split, c_hi = min(p.C, c_lo + p.c_per_split);
 #pragma unroll 1
     for (int c = c_lo; c < c_hi; ++c) {
