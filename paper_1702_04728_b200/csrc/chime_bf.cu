@@ -16,6 +16,7 @@
 #include "beamform_mma_kernel.cuh"
 #include "beamform_ws_kernel.cuh"
 #include "dedisperse_kernel.cuh"
+#include "umma_beamform_kernel.cuh"
 
 namespace {
 
@@ -62,6 +63,17 @@ struct chime_bf_plan {
     int host_parts = 1;                   // execute_host: frame ranges per channel
     uint8_t **d_peer_out = nullptr;       // execute_beam_major: device copy of the peers' receive-buffer pointers (<= 64)
     int32_t *d_delay = nullptr;   // [C][16] dedispersion delays of the last chime_bf_dedisperse call
+    // tensor-core N-S path (umma_beamform_kernel.cuh; upchan_len 128, any zero_pad)
+    bool use_umma = false;
+    uint32_t *d_wq = nullptr;     // TMEM images of the three-digit integer weights, 3 MiB per channel
+    int4 *d_rowsum = nullptr;
+    float2 *d_beta = nullptr;     // [C][4] E-W phase step of beam e
+    float *d_inv_s2 = nullptr;    // [C]
+    double *d_wscale = nullptr;   // [C] S_c
+    float2 *d_gains = nullptr;    // [C][2048] device copy of the gains (nullptr = unit)
+    int32_t *d_J = nullptr;       // [C][256]
+    int *d_status = nullptr, *h_status = nullptr;   // mapped host word: which wait timed out (0 = none)
+    int max_clusters = 0;         // co-resident clusters of 4 (persistent grid)
 };
 
 namespace {
@@ -231,9 +243,82 @@ bool build_weight_tables(chime_bf_plan *pl, cudaStream_t st) {
     return upload_on(&pl->d_wp, wp, st);
 }
 
+// Tensor-core path: the E-W phase steps (a5) -- 32 bytes per channel, all a re-pointing of the E-W beams uploads.
+bool build_ew_table(chime_bf_plan *pl, cudaStream_t st) {
+    std::vector<float2> beta((size_t)pl->C * 4);
+    for (int c = 0; c < pl->C; ++c)
+        for (int e = 0; e < 4; ++e) {
+            const double ph = -2.0 * kPi * (pl->freq[c] * 1e6) * pl->d_cyl * std::sin(pl->ew_deg[e] * kPi / 180.0) / kC0;
+            beta[(size_t)c * 4 + e] = make_float2((float)std::cos(ph), (float)std::sin(ph));
+        }
+    return upload_on(&pl->d_beta, beta, st);
+}
+
+// Tensor-core path: gains (a2) x N-S phases (a3, a4) as two-digit 16-bit integers, built on the device in double.
+bool build_umma_weights(chime_bf_plan *pl, cudaStream_t st) {
+    const int C = pl->C;
+    std::vector<double> scale(C);
+    std::vector<float> inv_s2(C);
+    for (int c = 0; c < C; ++c) {
+        double gmax = pl->gains.empty() ? 1.0 : 0.0;
+        if (!pl->gains.empty())
+            for (int i = 0; i < 2048; ++i) {
+                const float *g = &pl->gains[((size_t)c * 2048 + i) * 2];
+                gmax = std::max(gmax, std::hypot((double)g[0], (double)g[1]));
+            }
+        const double S = gmax > 0 ? (double)chime4::kWMax / (gmax * (1.0 + 1e-9)) : 1.0;
+        scale[c] = S;
+        inv_s2[c] = (float)((65536.0 / S) * (65536.0 / S));   // the kernel sums in units of the top digit
+    }
+    if (!upload_on(&pl->d_wscale, scale, st) || !upload_on(&pl->d_inv_s2, inv_s2, st)) return false;
+    if (!upload_on(&pl->d_J, pl->J, st)) return false;
+    if (!pl->gains.empty()) {
+        std::vector<float2> g((size_t)C * 2048);
+        memcpy(g.data(), pl->gains.data(), g.size() * sizeof(float2));
+        if (!upload_on(&pl->d_gains, g, st)) return false;
+    }
+    if (!pl->d_wq) {
+        CUDA_TRY(cudaMalloc((void **)&pl->d_wq, (size_t)C * 16 * chime4::kWqWordsPerSet * sizeof(uint32_t)));
+        CUDA_TRY(cudaMalloc((void **)&pl->d_rowsum, (size_t)C * 16 * 128 * sizeof(int4)));
+    }
+    chime4::WeightParams wp;
+    wp.wq = pl->d_wq;
+    wp.rowsum = pl->d_rowsum;
+    wp.gains = pl->gains.empty() ? nullptr : pl->d_gains;
+    wp.J = pl->d_J;
+    wp.turns = nullptr;
+    wp.scale = pl->d_wscale;
+    wp.NP = pl->NP;
+    chime4::build_weights_kernel<<<C * 16, 128, 0, st>>>(wp);
+    CUDA_TRY(cudaGetLastError());
+    return true;
+}
+
 bool build_tables(chime_bf_plan *pl) {
     const int NP = pl->use_mma ? 512 : pl->NP, U = pl->U;   // the tensor-core kernels always transform 512 points
-    if (!build_index_tables(pl, nullptr) || !build_weight_tables(pl, nullptr)) return false;
+    if (!build_index_tables(pl, nullptr)) return false;
+    if (pl->use_umma) {
+        std::vector<float2> tw128(128);
+        for (int k = 0; k < 128; ++k) {
+            const double a = -2.0 * kPi * (double)k / 128.0;
+            tw128[k] = make_float2((float)std::cos(a), (float)std::sin(a));
+        }
+        CUDA_TRY(cudaMemcpyToSymbol(chime2::c_tw128, tw128.data(), sizeof(float2) * 128));
+        CUDA_TRY(cudaFuncSetAttribute(chime4::umma_beamform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, chime4::kSmemBytes));
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(4 * 148);
+        cfg.blockDim = dim3(chime4::kThreads);
+        cfg.dynamicSmemBytes = chime4::kSmemBytes;
+        CUDA_TRY(cudaOccupancyMaxActiveClusters(&pl->max_clusters, chime4::umma_beamform_kernel, &cfg));
+        if (pl->max_clusters < 1) { set_err("plan_create: no cluster of 4 CTAs fits on this device"); return false; }
+        CUDA_TRY(cudaHostAlloc((void **)&pl->h_status, 128 * sizeof(int), cudaHostAllocMapped));   // survives a trapped kernel
+        memset(pl->h_status, 0, 128 * sizeof(int));
+        CUDA_TRY(cudaHostGetDevicePointer((void **)&pl->d_status, pl->h_status, 0));
+        CUDA_TRY(cudaMalloc((void **)&pl->d_delay, (size_t)pl->C * 16 * sizeof(int32_t)));
+        CUDA_TRY(cudaMalloc((void **)&pl->d_peer_out, 64 * sizeof(uint8_t *)));
+        return build_ew_table(pl, nullptr) && build_umma_weights(pl, nullptr);
+    }
+    if (!build_weight_tables(pl, nullptr)) return false;
     std::vector<float2> tw_np(NP), tw_u(U);
     for (int k = 0; k < NP; ++k) {
         const double a = -2.0 * kPi * (double)k / (double)NP;
@@ -332,6 +417,38 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
     kp.qscale = pl->norm * pl->scale;
     kp.qoffset = pl->offset;
     cudaStream_t st = (cudaStream_t)stream;
+    if (pl->use_umma) {
+        chime4::Params up;
+        up.in = in;
+        up.out_u8 = out_u8;
+        up.out_f32 = out_f32;
+        up.wq = pl->d_wq;
+        up.rowsum = pl->d_rowsum;
+        up.beta = pl->d_beta;
+        up.inv_s2 = pl->d_inv_s2;
+        up.n_time = pl->T;
+        up.n_frames = pl->R;
+        up.chan0 = chan0;
+        up.n_chan = n_chan;
+        up.frame0 = frame0;
+        up.n_frames_launch = n_fr;
+        up.peer_out = peer_out;
+        up.n_peers = n_peers;
+        up.chan_global0 = chan_global0;
+        up.norm = pl->norm;
+        up.scale = pl->scale;
+        up.offset = pl->offset;
+        up.status = pl->d_status;
+        const long long n_items = (long long)n_chan * ((n_fr + chime4::kChunkFrames - 1) / chime4::kChunkFrames) * 2;
+        const int n_cl = (int)std::min<long long>(n_items, pl->max_clusters);
+        chime4::umma_beamform_kernel<<<4 * n_cl, chime4::kThreads, chime4::kSmemBytes, st>>>(up);
+        const cudaError_t e4 = cudaGetLastError();
+        if (e4 != cudaSuccess) {
+            set_err("kernel launch failed: %s", cudaGetErrorString(e4));
+            return CHIME_BF_E_CUDA;
+        }
+        return CHIME_BF_OK;
+    }
     if (pl->use_mma) {
         chime2::Params mp;
         mp.in = in;
@@ -461,10 +578,11 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     pl->norm = (float)(1.0 / (256.0 * 4.0 * (double)p.upchan_len));
     {
         const char *kv = getenv("CHIME_BF_KERNEL");   // A/B switch: v1 generic, v2 block-synchronous mma, v3 warp-specialised (default)
-        pl->use_ws = !kv || !strcmp(kv, "v3");
+        pl->use_ws = !kv || !strcmp(kv, "v3") || !strcmp(kv, "v4");
     }
-    pl->n_pass = (p.zero_pad == 1024 && p.upchan_len == 128 && pl->use_ws) ? 2 : 1;
-    pl->use_mma = ((p.zero_pad == 512 || p.zero_pad == 256 || pl->n_pass == 2) && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1"));
+    pl->use_umma = p.upchan_len == 128 && getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v4");   // development switch, goes when v4 wins
+    pl->n_pass = (p.zero_pad == 1024 && p.upchan_len == 128 && pl->use_ws && !pl->use_umma) ? 2 : 1;
+    pl->use_mma = ((p.zero_pad == 512 || p.zero_pad == 256 || pl->n_pass == 2) && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1")) && !pl->use_umma;
     cudaGetDevice(&pl->device);
     pl->fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
     pl->d_feed = p.feed_spacing_m > 0 ? p.feed_spacing_m : 0.3048;
@@ -603,12 +721,14 @@ int chime_bf_update_gains(chime_bf_plan *pl, void *stream, const float *gains) {
     if (!pl) { set_err("update_gains: null plan"); return CHIME_BF_E_INVALID_ARG; }
     if (gains) pl->gains.assign(gains, gains + (size_t)pl->C * 2048 * 2);
     else pl->gains.clear();
+    if (pl->use_umma) return build_umma_weights(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
     return build_weight_tables(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
 }
 
 int chime_bf_update_ew_angles(chime_bf_plan *pl, void *stream, const double *ew_angles_deg) {
     if (!pl || !ew_angles_deg) { set_err("update_ew_angles: null argument"); return CHIME_BF_E_INVALID_ARG; }
     for (int e = 0; e < 4; ++e) pl->ew_deg[e] = ew_angles_deg[e];
+    if (pl->use_umma) return build_ew_table(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
     return build_weight_tables(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
 }
 
@@ -625,7 +745,9 @@ int chime_bf_update_pointings(chime_bf_plan *pl, void *stream, double f_ref_mhz,
         pl->ns_sin.clear();
         if (f_ref_mhz > 0) pl->fref = f_ref_mhz;
     }
-    return build_index_tables(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
+    if (!build_index_tables(pl, (cudaStream_t)stream)) return CHIME_BF_E_CUDA;
+    if (pl->use_umma) return build_umma_weights(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
+    return CHIME_BF_OK;
 }
 
 int chime_bf_dedisp_delays(const chime_bf_plan *pl, double dm, double f_ref_mhz, int32_t *host_out, int *n_out) {
@@ -719,6 +841,14 @@ int chime_bf_debug_unpack(chime_bf_plan *plan, void *stream, const uint8_t *in_u
     return CHIME_BF_OK;
 }
 
+int chime_bf_debug_status(const chime_bf_plan *plan, int code) { return (plan && plan->h_status && code >= 0 && code < 128) ? plan->h_status[code] : 0; }
+
+#ifdef CHIME_PROF
+int chime_bf_debug_prof(long long *host_out) {   // development builds only: per-warp wait cycles of the last launch
+    return cudaMemcpyFromSymbol(host_out, chime4::g_prof, sizeof(long long) * 148 * 4 * 24 * 12) == cudaSuccess ? 0 : -1;
+}
+#endif
+
 int chime_bf_n_frames(const chime_bf_plan *plan) { return plan ? plan->R : 0; }
 size_t chime_bf_in_bytes(const chime_bf_plan *plan) {
     return plan ? (size_t)plan->C * plan->T * 2048 : 0;
@@ -740,6 +870,14 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_stage_out);
     cudaFree(pl->d_delay);
     cudaFree(pl->d_peer_out);
+    cudaFree(pl->d_wq);
+    cudaFree(pl->d_rowsum);
+    cudaFree(pl->d_beta);
+    cudaFree(pl->d_inv_s2);
+    cudaFree(pl->d_wscale);
+    cudaFree(pl->d_gains);
+    cudaFree(pl->d_J);
+    if (pl->h_status) cudaFreeHost(pl->h_status);
     for (cudaEvent_t ev : pl->copy_done)
         if (ev) cudaEventDestroy(ev);
     if (pl->entry) cudaEventDestroy(pl->entry);

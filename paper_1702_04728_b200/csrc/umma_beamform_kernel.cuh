@@ -1,0 +1,785 @@
+// Fourth-generation fused CHIME/FRB beamformer kernel for sm_100a: the N-S transform (a3 + a4, with the gains a2
+// folded in) runs on the 5th-generation tensor cores as an exact integer GEMM (tcgen05.mma kind::i8), the E-W sum (a5)
+// is an all-to-all over distributed shared memory inside a cluster of 4 CTAs, and the time transform (a7), detection,
+// integration and quantisation (a8-a10) run on the FP32 pipe around it.  upchan_len = 128, any zero_pad (the padding
+// factor only changes the weights).  PAPER.md:51-53 (the three kernels), :59-61 (N-S transform), :84-86 (up-channelise).
+//
+// Mathematics.  All operators before |.|^2 are linear and act on different axes, so they commute:
+//   1. time, first stage, on the raw 4-bit integers (exact, packed four feeds per register): with t = u' + 16 k,
+//        S[8 q' + rho] = sum_{u'<16} W_16^{q'u'} W_128^{rho u'} A_rho[u'],   A_rho[u'] = sum_{k<8} x[u' + 16 k] W_8^{rho k}
+//      A_rho = E_rho + W_8^rho O_rho (even / odd taps).  Even rho: A_rho is a Gaussian integer, |re|,|im| <= 64.
+//      Odd rho: A_rho = E + O'/sqrt2, A_{rho+4} = E - O'/sqrt2 with E, O' = (+-1 - i) O Gaussian integers; E and O'
+//      go through the GEMM separately and are combined in fp32.
+//   2. N-S (+ gains, + bin selection): Y[m] = sum_n (g[n] W_NP^{J[m] n}) a[n] for a = A_rho[u'] (or E, O'): one row of
+//      a [256 beams x 2] x [256 feeds x 2] real matrix per (channel, pol, cylinder), the same for every column a.
+//      Weights = round(S_c * value) as 16-bit integers split into two signed 8-bit digits (256 hi + lo) that stay
+//      resident in TENSOR MEMORY (128 lanes = 128 beams, 2 x 128 columns = K 512 x 2 digits); the data columns are
+//      unsigned bytes (value + bias) in shared memory; two s32 accumulators (hi, lo) per output, recombined exactly in
+//      fp32 (256 hi + lo, bias * rowsum removed in the integer domain).  Real and imaginary outputs of a beam come
+//      from the SAME weight row [Wr | -Wi] applied to two variants of the data column, [re | im] and [im | -re], so
+//      both land in the same TMEM lane (= thread) in different columns.
+//   3. time, second stage, per cylinder (thread <-> beam, 16 values in registers): twiddle W_128^{rho u'}, FFT-16.
+//   4. E-W: Z_e = sum_cyl beta_e^cyl S_cyl (Horner), after an all-to-all by beam quarter over DSMEM: CTA r of the
+//      cluster owns cylinder r on the way in and beams 32 r .. 32 r + 31 of the tile on the way out.
+//   5. |Z|^2, sum over the 8 bins of a fine channel (= over rho), the 2 polarisations and the 3 blocks; quantise.
+//
+// Work decomposition: item = (channel, tile of 128 beams, chunk of up to 4 output frames), handed round-robin to the
+// clusters of a persistent grid.  Within an item the cluster runs polarisation 0 then 1 (weights reloaded in between)
+// and keeps the 4 frames' intensities in registers.  Per (block of 128 samples, pol) a CTA stages the raw 32 KiB of its
+// cylinder once (cp.async, XOR-swizzled) and makes 4 tiles from it (residue pairs {0,4}, {2,6}, {1,5}, {3,7}), each
+// a 128 x 64 x 512 x 2-digit GEMM (32 tcgen05.mma of K = 32) into one of two TMEM accumulator stages.
+//
+// Warp roles (768 threads, 1 CTA / SM):
+//   warps 0-1     MMA issuers (one lane each: hi / lo digit)  warps 2-3    raw-block stagers (cp.async -> mbarrier)
+//   warps 4-7     operand preparation (integer butterflies -> K-major B tile), weight loads into TMEM
+//   warps 8-15    accumulator drain (tcgen05.ld), digit recombination, combine, twiddle, FFT-16, DSMEM send;
+//                 warps 8-11 take even tiles, 12-15 odd tiles; warp % 4 = TMEM lane quarter = destination CTA
+//   warps 16-23   receive side: E-W Horner, detect, accumulate; item epilogue (normalise, quantise, store)
+// All hand-overs are mbarriers (local, or remote through mapa for the two cluster-level ones).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "beamform_kernel.cuh"       // chime::beam_major_dst
+#include "beamform_mma_kernel.cuh"   // chime2::int_bfly4, time_pretwiddle, c_tw128
+#include "fft_regs.cuh"
+
+namespace chime4 {
+
+using chime::bitrev;
+using chime::fft_dif;
+
+constexpr int kThreads = 768;
+constexpr int kChunkFrames = 4;                 // output frames per item (their intensities live in registers)
+constexpr int kRawBytes = 128 * 256;            // one (block, pol, cylinder): 32 KiB
+constexpr int kBopBytes = 64 * 512;             // one B tile: 64 columns x K 512 bytes
+constexpr int kRecvBytes = 4 * 2 * 8 * 32 * 16; // one receive slot: [cyl][res][i pair][beam][2 x float2] = 32 KiB
+constexpr int kOfsRaw = 0, kOfsBop = 2 * kRawBytes, kOfsRecv = kOfsBop + 2 * kBopBytes;
+constexpr int kOfsOut = kOfsRecv + 2 * kRecvBytes;
+constexpr int kOutBytes = 4 * 32 * 17 * 4;      // [e][beam][16 + 1 pad] floats
+constexpr int kOfsBar = kOfsOut + kOutBytes;
+// mbarrier indices
+enum { B_RAW_FULL = 0, B_RAW_EMPTY = 2, B_BOP_FULL = 4, B_BOP_EMPTY = 6, B_TM_FULL = 8, B_TM_EMPTY = 10,
+       B_RECV_FULL = 12, B_SLOT_FREE = 14 /* [dest 4][slot 2] */, B_W_FREE = 22, B_W_READY = 23,
+       B_ACC_FULL = 24 /* [group 2][slot 2] */, B_ACC_EMPTY = 28, B_COUNT = 32 };
+constexpr int kSmemBytes = kOfsBar + B_COUNT * 8 + 16;
+
+constexpr int kDigits = 3;                      // signed 8-bit digits per weight (24-bit weights)
+constexpr int kWCols = 128 * kDigits;           // TMEM columns of the stationary weights
+constexpr size_t kWqWordsPerSet = 128 * kWCols; // one (channel, pol, cyl, tile): 128 rows x 384 TMEM columns
+
+struct Params {
+    const uint8_t *in;        // [C][T][2048]
+    uint8_t *out_u8;          // [C][R][4][256][16]
+    float *out_f32;           // same layout, or nullptr
+    const uint32_t *wq;       // [C][pol 2][cyl 4][tile 2][quarter 4][c32 12][i 32][lane 32]: TMEM images of the weights
+    const int4 *rowsum;       // [C][pol][cyl][tile][128] sum of the digits of each row (digit 2, 1, 0, unused)
+    const float2 *beta;       // [C][4] E-W phase step per cylinder of beam e
+    const float *inv_s2;      // [C] 1 / S_c^2 (weight scale)
+    int n_time, n_frames;
+    int chan0, n_chan;        // channel range of this launch
+    int frame0, n_frames_launch;
+    uint8_t *const *peer_out; // beam-major exchange (chime::beam_major_dst), nullptr = off
+    int n_peers, chan_global0;
+    float norm, scale, offset;
+    int *status;              // set to non-zero when a wait timed out (the kernel traps afterwards)
+};
+
+// ---- PTX wrappers ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t a, uint32_t n) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(a), "r"(n) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t a) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(a) : "memory");
+}
+// "I have finished reading" to a peer CTA (ra from mapa).  Relaxed: the loads it protects have already delivered their
+// values to the arithmetic that precedes it; a release at cluster scope here costs hundreds of cycles per arrive.
+__device__ __forceinline__ void mbar_arrive_remote_relaxed(uint32_t ra) {
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" :: "r"(ra) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t a, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(a), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ uint32_t mapa(uint32_t a, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
+    return r;
+}
+template <bool CLUSTER>
+__device__ __forceinline__ bool mbar_try(uint32_t a, uint32_t parity) {
+    uint32_t ok;
+    if constexpr (CLUSTER)
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    else
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    return ok != 0;
+}
+// Waits for the phase of parity `parity` to complete.  A wait that lasts ~2 s is a protocol bug: flag it and trap
+// instead of hanging the GPU.
+#ifdef CHIME_PROF
+__device__ long long g_prof[148 * 4][24][12];
+#define PW(code, stmt) { const long long _t = clock64(); stmt; prof_w[code] += clock64() - _t; }
+#else
+#define PW(code, stmt) { stmt; }
+#endif
+template <bool CLUSTER = false>
+__device__ __forceinline__ void mbar_wait(uint32_t a, uint32_t parity, int *status, int code, uint32_t info = 0) {
+    if (mbar_try<CLUSTER>(a, parity)) return;
+    const long long t0 = clock64();
+
+    while (!mbar_try<CLUSTER>(a, parity)) {
+        if (clock64() - t0 > 2000000000ll) {
+            atomicCAS(status + code * 8 + (blockIdx.x & 7), 0, 1 | ((int)(threadIdx.x >> 5) << 8) | ((int)info << 16));
+            __threadfence_system();
+            for (long long t1 = clock64(); clock64() - t1 < 1500000000ll;) {}
+            __trap();
+        }
+    }
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem descriptor], kind::i8
+template <bool ACC>
+__device__ __forceinline__ void umma_i8_ts(uint32_t d, uint32_t a, uint64_t bdesc, uint32_t idesc) {
+    if constexpr (ACC)
+        asm volatile("{ .reg .pred p; setp.eq.u32 p, 1, 1; tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p; }"
+                     :: "r"(d), "r"(a), "l"(bdesc), "r"(idesc) : "memory");
+    else
+        asm volatile("{ .reg .pred p; setp.eq.u32 p, 1, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p; }"
+                     :: "r"(d), "r"(a), "l"(bdesc), "r"(idesc) : "memory");
+}
+// K-major, no swizzle: core matrix = 8 rows x 16 bytes (128 contiguous bytes); lbo = byte distance of the K-adjacent
+// core matrix, sbo = of the next 8 rows; descriptor version 1 (sm_100).
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) |
+           ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | (1ull << 46);
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t *v) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t *v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+                 "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+                 "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+                 :: "r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+                    "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
+                    "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
+                    "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+                 : "memory");
+}
+// One lane of a converged warp (elect.sync): ptxas then knows that a single thread issues what follows and moves the
+// operands of the tcgen05 instructions to uniform registers once, instead of looping over the active lanes.
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{ .reg .pred p; elect.sync _|p, 0xffffffff; selp.u32 %0, 1, 0, p; }" : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ void bar_sync_named(int id, int n) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(n) : "memory"); }
+
+// ---- a1: the nibble split of the packed baseband, four inputs per register ---------------------------------------
+// byte = ((re + 8) << 4) | (im + 8)  ->  offset-binary real parts and imaginary parts, one per byte
+__device__ __forceinline__ void split_nibbles(uint32_t w, uint32_t &re_off, uint32_t &im_off) {
+    re_off = (w >> 4) & 0x0F0F0F0Fu;
+    im_off = w & 0x0F0F0F0Fu;
+}
+
+// ---- operand preparation: one tile (residue pair) of one raw block ----------------------------------------------
+// TT = 0: columns A_0, A_4; 1: A_2, A_6; 2: E_1, O'_1; 3: E_3, O'_3.  B tile row n = 32 variant + 16 set + u',
+// K byte 32 j + i (i < 16): first half of feed 16 j + i, 32 j + 16 + i: second half; variant 0 = [re | im],
+// variant 1 = [im | -re]; signed bytes (the packed butterflies run on biased bytes, bias 64 (A, O') or 32 (E), which is
+// removed at the end).  Layout [kc = K/16][row group 8][8 rows][16 B].
+template <int TT>
+__device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned char *bop, const int pw, const int lane) {
+    constexpr int R4 = (TT == 0) ? 0 : (TT == 1) ? 2 : (TT == 2) ? 1 : 3;
+    constexpr uint32_t H40 = 0x40404040u, H80 = 0x80808080u;
+    const int j = 4 * pw + (lane >> 3);                 // 16-feed chunk
+    const int x7 = lane & 7;
+    const unsigned char *src = raw + (j >> 3) * 16384 + (((j & 7) ^ x7) << 4);
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const int up = x7 + 8 * it;                     // u'
+        uint4 q[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) q[k] = *reinterpret_cast<const uint4 *>(src + (up + 16 * k) * 128);
+        uint32_t re0[4], im0[4], ng0[4], re1[4], im1[4], ng1[4];
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            uint32_t t[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) t[k] = w == 0 ? q[k].x : w == 1 ? q[k].y : w == 2 ? q[k].z : q[k].w;
+            uint32_t er, ei, orr, oi;
+            chime2::int_bfly4<R4>(t[0], t[2], t[4], t[6], er, ei);     // bytes = value + 32
+            chime2::int_bfly4<R4>(t[1], t[3], t[5], t[7], orr, oi);
+            if constexpr (TT == 0) {          // A_0 = E + O, A_4 = E - O
+                re0[w] = er + orr;          im0[w] = ei + oi;
+                re1[w] = (er + H40) - orr;  im1[w] = (ei + H40) - oi;
+                ng0[w] = H80 - re0[w];      ng1[w] = H80 - re1[w];
+            } else if constexpr (TT == 1) {   // A_2 = E + (-i) O, A_6 = E - (-i) O;  (-i)(a + i b) = b - i a
+                re0[w] = er + oi;           im0[w] = (ei + H40) - orr;
+                re1[w] = (er + H40) - oi;   im1[w] = ei + orr;
+                ng0[w] = H80 - re0[w];      ng1[w] = H80 - re1[w];
+            } else if constexpr (TT == 2) {   // E_1 (bias 32), O' = (1 - i) O = (a + b) + i (b - a)
+                re0[w] = er;                im0[w] = ei;
+                re1[w] = orr + oi;          im1[w] = (oi + H40) - orr;
+                ng0[w] = H40 - re0[w];      ng1[w] = H80 - re1[w];
+            } else {                          // E_3 (bias 32), O' = (-1 - i) O = (b - a) - i (a + b)
+                re0[w] = er;                im0[w] = ei;
+                re1[w] = (oi + H40) - orr;  im1[w] = H80 - (orr + oi);
+                ng0[w] = H40 - re0[w];      ng1[w] = H80 - re1[w];
+            }
+        }
+        // biased bytes (value + bias <= 128) -> two's complement bytes: (b + 128 - bias) ^ 0x80, no carry between bytes
+        constexpr uint32_t C0 = (TT < 2) ? 0x40404040u : 0x60606060u, C1 = 0x40404040u;
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            re0[w] = (re0[w] + C0) ^ H80;  im0[w] = (im0[w] + C0) ^ H80;  ng0[w] = (ng0[w] + C0) ^ H80;
+            re1[w] = (re1[w] + C1) ^ H80;  im1[w] = (im1[w] + C1) ^ H80;  ng1[w] = (ng1[w] + C1) ^ H80;
+        }
+        // rows: variant 0 set s: 16 s + u';  variant 1: 32 + 16 s + u'.  (row >> 3) * 128 + (row & 7) * 16
+        unsigned char *d = bop + (2 * j) * 1024 + it * 128 + x7 * 16;
+        *reinterpret_cast<uint4 *>(d) = make_uint4(re0[0], re0[1], re0[2], re0[3]);                 // v0 set0, first half
+        *reinterpret_cast<uint4 *>(d + 1024) = make_uint4(im0[0], im0[1], im0[2], im0[3]);          //          second
+        *reinterpret_cast<uint4 *>(d + 256) = make_uint4(re1[0], re1[1], re1[2], re1[3]);           // v0 set1
+        *reinterpret_cast<uint4 *>(d + 256 + 1024) = make_uint4(im1[0], im1[1], im1[2], im1[3]);
+        *reinterpret_cast<uint4 *>(d + 512) = make_uint4(im0[0], im0[1], im0[2], im0[3]);           // v1 set0
+        *reinterpret_cast<uint4 *>(d + 512 + 1024) = make_uint4(ng0[0], ng0[1], ng0[2], ng0[3]);
+        *reinterpret_cast<uint4 *>(d + 768) = make_uint4(im1[0], im1[1], im1[2], im1[3]);           // v1 set1
+        *reinterpret_cast<uint4 *>(d + 768 + 1024) = make_uint4(ng1[0], ng1[1], ng1[2], ng1[3]);
+    }
+}
+
+// ---- accumulator drain: one digit pass (64 s32 columns of this thread's lane) folded into 64 fp32 partial sums ------
+// Every accumulator column STARTS from the bit pattern of 1.5 * 2^23 (written by the previous drain), so what comes out
+// is already the float M + a (|a| < 2^22, exact): y = a2 + a1 / 256 + a0 / 65536 in units of the top digit costs one
+// instruction per value and pass.  Column n = 32 variant + 16 set + u'.
+constexpr uint32_t kMagicBits = 0x4B400000u;               // 1.5 * 2^23 = 12582912
+constexpr float kMagicSum = 12582912.0f + 49152.0f + 192.0f;   // M (1 + 2^-8 + 2^-16), an exact integer < 2^24
+
+__device__ __forceinline__ void tmem_fill16(uint32_t taddr, uint32_t v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1};"
+                 :: "r"(taddr), "r"(v) : "memory");
+}
+
+template <int P>
+__device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64]) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        uint32_t h[16];
+        tmem_ld16(tslot + 16 * c, h);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        tmem_fill16(tslot + 16 * c, kMagicBits);             // ready for the slot's next pass
+#pragma unroll
+        for (int i = 0; i < 16; i += 2) {
+            const float2 f = make_float2(__uint_as_float(h[i]), __uint_as_float(h[i + 1]));
+            float2 r;
+            if constexpr (P == 0) r = __fadd2_rn(f, make_float2(-kMagicSum, -kMagicSum));
+            else if constexpr (P == 1) r = __ffma2_rn(f, make_float2(1.0f / 256.0f, 1.0f / 256.0f), make_float2(y[16 * c + i], y[16 * c + i + 1]));
+            else r = __ffma2_rn(f, make_float2(1.0f / 65536.0f, 1.0f / 65536.0f), make_float2(y[16 * c + i], y[16 * c + i + 1]));
+            y[16 * c + i] = r.x;
+            y[16 * c + i + 1] = r.y;
+        }
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+
+template <int RHO>
+__device__ __forceinline__ void twiddle_fft16(float2 (&a)[16]) {
+    if constexpr (RHO != 0) chime2::time_pretwiddle<RHO, 1>(a);
+    fft_dif<16>(a);
+}
+
+// a: 16 FFT outputs (index i = bin bitrev(i)) of residue `res` -> receive slot of the destination CTA
+// The stores are asynchronous and each one reports its 16 bytes to the destination's mbarrier (complete_tx), so the
+// receiver's wait on that barrier is the only synchronisation: no fence, no arrive on the sending side.
+__device__ __forceinline__ void send16(uint32_t rslot, uint32_t rbar, int cyl, int res, int lane, const float2 (&a)[16]) {
+#pragma unroll
+    for (int ip = 0; ip < 8; ++ip) {
+        const uint32_t addr = rslot + (uint32_t)((((cyl * 2 + res) * 8 + ip) * 32 + lane) * 16);
+        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1,%2,%3,%4}, [%5];"
+                     :: "r"(addr), "f"(a[2 * ip].x), "f"(a[2 * ip].y), "f"(a[2 * ip + 1].x), "f"(a[2 * ip + 1].y), "r"(rbar) : "memory");
+    }
+}
+
+// One tile on the drain side: the three digit passes arrive one after the other in the two rotating accumulator
+// slots (pass 3 tau + p uses slot (tau + p) & 1; n_use counts this group's uses of each slot = the phase of its
+// barriers); each pass is folded into y and the slot handed back at once.
+template <int TT>
+__device__ __forceinline__ void epi_tile(const uint32_t tlane, const uint32_t bar_full0, const uint32_t bar_empty0,
+                                         uint32_t (&n_use)[2], const uint32_t tau, const uint32_t rslot, const uint32_t rbar,
+                                         const int cyl, const int lane, const uint32_t slot_free_bar,
+                                         const uint32_t sf_parity, int *status, long long *prof_w) {
+    float y[64];
+#pragma unroll
+    for (int p = 0; p < 3; ++p) {
+        const uint32_t slot = (tau + p) & 1;     // = (3 tau + p) & 1
+        PW(9, mbar_wait(bar_full0 + 8 * slot, n_use[slot] & 1, status, 9, tau);)
+        ++n_use[slot];
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t tslot = tlane + kWCols + 64 * slot;
+        PW(6, if (p == 0) drain_pass<0>(tslot, y);
+        else if (p == 1) drain_pass<1>(tslot, y);
+        else drain_pass<2>(tslot, y);)
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty0 + 8 * slot);   // the slot is in registers: hand it back to the issuer
+    }
+    float2 a0[16], a1[16];
+#ifdef CHIME_PROF
+    const long long t_fft = clock64();
+#endif
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+        a0[u] = make_float2(y[u], y[32 + u]);
+        a1[u] = make_float2(y[16 + u], y[48 + u]);
+    }
+    if constexpr (TT >= 2) {   // A_rho = E + O'/sqrt2, A_{rho+4} = E - O'/sqrt2
+        constexpr float s = 0.70710678118654752440f;
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            const float2 e = a0[u], o = a1[u];
+            a0[u] = __ffma2_rn(o, make_float2(s, s), e);
+            a1[u] = __ffma2_rn(o, make_float2(-s, -s), e);
+        }
+    }
+    constexpr int RHO = (TT == 0) ? 0 : (TT == 1) ? 2 : (TT == 2) ? 1 : 3;
+    twiddle_fft16<RHO>(a0);
+    twiddle_fft16<RHO + 4>(a1);
+#ifdef CHIME_PROF
+    prof_w[7] += clock64() - t_fft;
+#endif
+    PW(5, mbar_wait(slot_free_bar, sf_parity, status, 5);)     // the destination has consumed this slot's previous tile
+    PW(8, send16(rslot, rbar, cyl, 0, lane, a0);
+    send16(rslot, rbar, cyl, 1, lane, a1);)
+}
+
+__global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_beamform_kernel(const Params prm) {
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    const int cluster_id = blockIdx.x >> 2, n_clusters = gridDim.x >> 2;
+    const uint32_t bar0 = smem_u32(smem + kOfsBar);
+    auto BAR = [&](int i) { return bar0 + 8u * (uint32_t)i; };
+    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(smem + kOfsBar + B_COUNT * 8);
+
+    if (tid == 0) {
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(BAR(B_RAW_FULL + s), 64);
+            mbar_init(BAR(B_RAW_EMPTY + s), 4);
+            mbar_init(BAR(B_BOP_FULL + s), 4);
+            mbar_init(BAR(B_BOP_EMPTY + s), 2);
+            mbar_init(BAR(B_RECV_FULL + s), 1);
+        }
+        for (int i = 0; i < 8; ++i) mbar_init(BAR(B_SLOT_FREE + i), 8);
+        for (int i = 0; i < 4; ++i) {
+            mbar_init(BAR(B_ACC_FULL + i), 1);    // accumulator slot, per drain group: one commit per digit pass
+            mbar_init(BAR(B_ACC_EMPTY + i), 4);   // ... drained by the 4 warps of the group
+        }
+        mbar_init(BAR(B_W_FREE), 2);
+        mbar_init(BAR(B_W_READY), 4);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_expect_tx(BAR(B_RECV_FULL + 0), kRecvBytes);   // every receive slot expects one tile = 32 KiB of st.async
+        mbar_expect_tx(BAR(B_RECV_FULL + 1), kRecvBytes);
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(s_tmem)), "n"(512) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    // every CTA's barriers exist before any remote arrive
+    asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory");
+    const uint32_t tb = *s_tmem;
+
+    const int n_chunks = (prm.n_frames_launch + kChunkFrames - 1) / kChunkFrames;
+    const int n_items = prm.n_chan * n_chunks * 2;
+    int *const status = prm.status;
+    long long prof_w[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    const long long prof_t0 = clock64();
+    (void)prof_t0;
+
+#define ITEM_LOOP                                                                          \
+    for (int item = cluster_id; item < n_items; item += n_clusters) {                      \
+        const int rt = item & 1, chunk = (item >> 1) % n_chunks;                           \
+        const int c = prm.chan0 + (item >> 1) / n_chunks;                                  \
+        const int fr0 = prm.frame0 + chunk * kChunkFrames;                                 \
+        const int nf = min(kChunkFrames, prm.frame0 + prm.n_frames_launch - fr0);          \
+        (void)rt; (void)c; (void)fr0; (void)nf;
+
+    // Register budget per warpgroup: 32 / 80 / 120 / 120 / 64 / 64.  setmaxnreg only redistributes what the CTA was
+    // launched with (768 x 80), so the six budgets must not add up to more than 6 x 80.
+    if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
+    else if (warp >= 16) asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
+    else if (warp >= 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 120;");
+
+    if (warp < 2) {
+        // ============================== MMA issuers: warp w owns accumulator slot w ==============================
+        // Digit pass pi = 3 tau + p of tile tau goes to slot pi & 1 (two 64-column slots rotate under the three passes:
+        // weights 384 + accumulators 128 = all 512 columns).  D = s32, A = s8, B = s8, K-major, N = 64, M = 128.  Every
+        // pass ACCUMULATES onto what the last drain left in the slot (the magic constant, see drain_pass).
+        constexpr uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
+        // Slot barriers are kept per drain group (g = tau & 1), so that every waiter sees the phases of its barrier in
+        // order; the issuer waits for the drain of the slot's PREVIOUS use, whichever group that was.
+        const uint32_t myslot = warp;
+        uint32_t tau = 0, seg = 0;
+        uint32_t n_use[2] = {1, 0};     // drains of my slot requested so far, per group (group 0's initial fill counts)
+        int prev_g = 0;                 // group that drains (fills) my slot before my next pass
+        ITEM_LOOP
+            for (int pol = 0; pol < 2; ++pol) {
+                PW(1, mbar_wait(BAR(B_W_READY), seg & 1, status, 1, seg);)
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const int ntiles = nf * 12;
+                for (int t = 0; t < ntiles; ++t, ++tau) {
+                    const uint32_t s = tau & 1, ph = (tau >> 1) & 1;
+                    PW(2, mbar_wait(BAR(B_BOP_FULL + s), ph, status, 2, tau);)
+                    const uint64_t bd0 = make_desc(smem_u32(smem + kOfsBop) + s * kBopBytes, 1024, 128);
+#pragma unroll 1
+                    for (uint32_t p = 0; p < 3; ++p) {
+                        const uint32_t pi = 3 * tau + p;
+                        if ((pi & 1) != myslot) continue;
+                        const int g = tau & 1;
+                        PW(3, mbar_wait(BAR(B_ACC_EMPTY + 2 * prev_g + myslot), (n_use[prev_g] - 1) & 1, status, 3, tau);)
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                        if (elect_one()) {
+                            const uint32_t d = tb + kWCols + 64 * myslot;
+                            uint32_t a = tb + 128 * p;
+                            uint64_t bd = bd0;
+                            umma_i8_ts<true>(d, a, bd, idesc);
+#pragma unroll 1
+                            for (int k = 1; k < 16; ++k) {   // rolled: the issuers run on 32 registers
+                                a += 8;
+                                bd += 2048 >> 4;
+                                umma_i8_ts<true>(d, a, bd, idesc);
+                            }
+                            umma_commit(BAR(B_ACC_FULL + 2 * g + myslot));
+                        }
+                        __syncwarp();
+                        ++n_use[g];
+                        prev_g = g;
+                    }
+                    if (elect_one()) umma_commit(BAR(B_BOP_EMPTY + s));   // both issuers: the B tile is free when all 3 passes are done
+                    __syncwarp();
+                }
+                if (elect_one()) umma_commit(BAR(B_W_FREE));
+                __syncwarp();
+                ++seg;
+            }
+        }
+    } else if (warp < 4) {
+        // ============================== raw-block stagers ==============================
+        const int st = tid - 64;
+        uint32_t beta = 0;
+        ITEM_LOOP
+            for (int pol = 0; pol < 2; ++pol)
+                for (int fr = 0; fr < nf; ++fr)
+                    for (int blk = 0; blk < 3; ++blk, ++beta) {
+                        const uint32_t b = beta & 1;
+                        PW(4, mbar_wait(BAR(B_RAW_EMPTY + b), ((beta >> 1) & 1) ^ 1, status, 4, beta);)
+                        const size_t t0 = (size_t)((fr0 + fr) * 3 + blk) * 128;
+                        const uint8_t *src = prm.in + ((size_t)c * prm.n_time + t0) * 2048 + pol * 1024 + rank * 256;
+                        const uint32_t dst = smem_u32(smem + kOfsRaw) + b * kRawBytes;
+                        for (int idx = st; idx < 2048; idx += 64) {
+                            const int t = idx >> 4, j = idx & 15;
+                            const uint32_t d = dst + (j >> 3) * 16384 + t * 128 + (((j & 7) ^ (t & 7)) << 4);
+                            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(src + (size_t)t * 2048 + j * 16) : "memory");
+                        }
+                        asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" :: "r"(BAR(B_RAW_FULL + b)) : "memory");
+                    }
+        }
+        asm volatile("cp.async.wait_all;" ::: "memory");
+    } else if (warp < 8) {
+        // ============================== operand preparation + weight loads ==============================
+        const int pw = warp - 4;   // = TMEM lane quarter for the weight loads (warp % 4)
+        uint32_t tau = 0, seg = 0, beta = 0;
+        ITEM_LOOP
+            for (int pol = 0; pol < 2; ++pol) {
+                if (seg > 0) {
+                    PW(6, mbar_wait(BAR(B_W_FREE), (seg - 1) & 1, status, 6);)   // every MMA that read the old weights is done
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                }
+                {
+                    const uint32_t *wsrc = prm.wq + ((((size_t)c * 2 + pol) * 4 + rank) * 2 + rt) * kWqWordsPerSet + pw * (kWCols * 32) + lane;
+#pragma unroll 1
+                    for (int c32 = 0; c32 < kWCols / 32; ++c32) {
+                        uint32_t v[32];
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = __ldg(wsrc + c32 * 1024 + i * 32);
+                        tmem_st32(tb + ((uint32_t)(32 * pw) << 16) + 32 * c32, v);
+                    }
+                    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(BAR(B_W_READY));
+                }
+                ++seg;
+                for (int fr = 0; fr < nf; ++fr)
+                    for (int blk = 0; blk < 3; ++blk, ++beta) {
+                        const uint32_t b = beta & 1;
+                        PW(7, mbar_wait(BAR(B_RAW_FULL + b), (beta >> 1) & 1, status, 7, beta);)
+                        const unsigned char *raw = smem + kOfsRaw + b * kRawBytes;
+#pragma unroll 1
+                        for (int tt = 0; tt < 4; ++tt, ++tau) {
+                            const uint32_t s = tau & 1;
+                            PW(8, mbar_wait(BAR(B_BOP_EMPTY + s), ((tau >> 1) & 1) ^ 1, status, 8, tau);)
+                            unsigned char *bop = smem + kOfsBop + s * kBopBytes;
+                            switch (tt) {
+                                case 0: prep_tile<0>(raw, bop, pw, lane); break;
+                                case 1: prep_tile<1>(raw, bop, pw, lane); break;
+                                case 2: prep_tile<2>(raw, bop, pw, lane); break;
+                                default: prep_tile<3>(raw, bop, pw, lane); break;
+                            }
+                            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes -> tensor-core reads
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(BAR(B_BOP_FULL + s));
+                        }
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(BAR(B_RAW_EMPTY + b));
+                    }
+            }
+        }
+    } else if (warp < 16) {
+        // ============================== accumulator drain, FFT-16, DSMEM send ==============================
+        const int g = (warp - 8) >> 2, q = warp & 3;
+        const uint32_t tlane = tb + ((uint32_t)(32 * q) << 16);
+        const uint32_t rslot = mapa(smem_u32(smem + kOfsRecv) + g * kRecvBytes, q);
+        const uint32_t rfull = mapa(BAR(B_RECV_FULL + g), q);
+        const uint32_t sfree = BAR(B_SLOT_FREE + 2 * q + g);
+        const uint32_t accf = BAR(B_ACC_FULL + 2 * g), acce = BAR(B_ACC_EMPTY + 2 * g);
+        uint32_t n_use[2] = {0, 0};
+        uint32_t tau = 0;
+        if (g == 0) {   // both accumulator slots start from the magic constant: group 0's "drain number 0" of each slot
+#pragma unroll
+            for (int c = 0; c < 8; ++c) tmem_fill16(tlane + kWCols + 16 * c, kMagicBits);
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(acce);
+                mbar_arrive(acce + 8);
+            }
+        }
+        ITEM_LOOP
+            for (int pol = 0; pol < 2; ++pol) {
+                const int ntiles = nf * 12;
+#pragma unroll 1
+                for (int t = 0; t < ntiles; ++t, ++tau) {
+                    if ((int)(tau & 1) != g) continue;
+                    const uint32_t sfp = ((tau >> 1) & 1) ^ 1;
+#ifdef CHIME_PROF
+                    const long long t_tile = clock64();
+#endif
+                    switch (t & 3) {
+                        case 0: epi_tile<0>(tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, sfp, status, prof_w); break;
+                        case 1: epi_tile<1>(tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, sfp, status, prof_w); break;
+                        case 2: epi_tile<2>(tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, sfp, status, prof_w); break;
+                        default: epi_tile<3>(tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, sfp, status, prof_w); break;
+                    }
+#ifdef CHIME_PROF
+                    prof_w[10] += clock64() - t_tile;
+#endif
+                }
+            }
+        }
+    } else {
+        // ============================== receive side: E-W, detect, integrate, output ==============================
+        const int ip = warp - 16, rtid = tid - 512;
+        uint32_t sf_remote[4][2];
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            sf_remote[s][0] = mapa(BAR(B_SLOT_FREE + 2 * rank + 0), s);
+            sf_remote[s][1] = mapa(BAR(B_SLOT_FREE + 2 * rank + 1), s);
+        }
+        float *ost = reinterpret_cast<float *>(smem + kOfsOut);
+        const int g0 = (bitrev(2 * ip, 4) + 8) & 15, g1 = (bitrev(2 * ip + 1, 4) + 8) & 15;
+        uint32_t tau = 0;
+        ITEM_LOOP
+            float2 be[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) be[e] = __ldg(prm.beta + (size_t)c * 4 + e);
+            float acc[kChunkFrames][4][2];
+#pragma unroll
+            for (int f = 0; f < kChunkFrames; ++f)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) acc[f][e][0] = acc[f][e][1] = 0.f;
+#pragma unroll 1
+            for (int pol = 0; pol < 2; ++pol) {
+#pragma unroll
+                for (int fr = 0; fr < kChunkFrames; ++fr) {
+                    if (fr < nf) {
+#pragma unroll 1
+                        for (int t = 0; t < 12; ++t, ++tau) {
+                            const uint32_t s = tau & 1;
+                            PW(10, mbar_wait(BAR(B_RECV_FULL + s), (tau >> 1) & 1, status, 10, tau);)
+                            if (ip == 0 && lane == 0) mbar_expect_tx(BAR(B_RECV_FULL + s), kRecvBytes);   // arm the slot's next tile
+                            const unsigned char *base = smem + kOfsRecv + s * kRecvBytes + (ip * 32 + lane) * 16;
+#pragma unroll
+                            for (int res = 0; res < 2; ++res) {
+                                float4 sv[4];
+#pragma unroll
+                                for (int cy = 0; cy < 4; ++cy)
+                                    sv[cy] = *reinterpret_cast<const float4 *>(base + ((cy * 2 + res) * 8) * 512);
+#pragma unroll
+                                for (int e = 0; e < 4; ++e) {
+                                    // Horner in beta_e: z = s0 + b (s1 + b (s2 + b s3)), two points at once
+                                    const float2 bx = make_float2(be[e].x, be[e].x), by = make_float2(-be[e].y, be[e].y);
+                                    float2 za = make_float2(sv[3].x, sv[3].y), zb = make_float2(sv[3].z, sv[3].w);
+#pragma unroll
+                                    for (int cy = 2; cy >= 0; --cy) {
+                                        const float2 sa = make_float2(sv[cy].x, sv[cy].y), sb = make_float2(sv[cy].z, sv[cy].w);
+                                        const float2 ta = __ffma2_rn(za, bx, sa), tb2 = __ffma2_rn(zb, bx, sb);
+                                        za = __ffma2_rn(make_float2(za.y, za.x), by, ta);
+                                        zb = __ffma2_rn(make_float2(zb.y, zb.x), by, tb2);
+                                    }
+                                    acc[fr][e][0] = fmaf(za.x, za.x, fmaf(za.y, za.y, acc[fr][e][0]));
+                                    acc[fr][e][1] = fmaf(zb.x, zb.x, fmaf(zb.y, zb.y, acc[fr][e][1]));
+                                }
+                            }
+                            __syncwarp();
+                            if (lane == 0) {
+#pragma unroll
+                                for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc][s]);
+                            }
+                        }
+                    }
+                }
+            }
+            // ---- item epilogue: a9 normalise, a10 quantise, one 16-byte store per beam ----
+            const float nrm = prm.norm * __ldg(prm.inv_s2 + c);
+#pragma unroll
+            for (int fr = 0; fr < kChunkFrames; ++fr) {
+                if (fr < nf) {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        ost[(e * 32 + lane) * 17 + g0] = acc[fr][e][0] * nrm;
+                        ost[(e * 32 + lane) * 17 + g1] = acc[fr][e][1] * nrm;
+                    }
+                    bar_sync_named(1, 256);
+                    if (rtid < 128) {
+                        const int e = rtid >> 5, ns = 128 * rt + 32 * (int)rank + (rtid & 31);
+                        const int Rf = fr0 + fr;
+                        const float *v = ost + rtid * 17;
+                        const size_t ob = ((((size_t)c * prm.n_frames + Rf) * 4 + e) * 256 + ns) * 16;
+                        if (prm.out_f32 != nullptr) {
+                            float4 *dst = reinterpret_cast<float4 *>(prm.out_f32 + ob);
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) dst[k] = make_float4(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
+                        } else {
+                            uint32_t qw[4];
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                uint32_t word = 0;
+#pragma unroll
+                                for (int b = 0; b < 4; ++b) {
+                                    const float x = fmaf(v[4 * k + b], prm.scale, prm.offset);
+                                    word |= (uint32_t)__float2int_rn(fminf(fmaxf(x, 0.f), 255.f)) << (8 * b);
+                                }
+                                qw[k] = word;
+                            }
+                            const uint4 qv = make_uint4(qw[0], qw[1], qw[2], qw[3]);
+                            if (prm.peer_out != nullptr)
+                                *chime::beam_major_dst(prm.peer_out, prm.n_peers, prm.chan_global0 + c, prm.n_frames, Rf, e * 256 + ns) = qv;
+                            else
+                                *reinterpret_cast<uint4 *>(prm.out_u8 + ob) = qv;
+                        }
+                    }
+                    bar_sync_named(1, 256);
+                }
+            }
+        }
+    }
+#undef ITEM_LOOP
+#ifdef CHIME_PROF
+    if (lane == 0) {
+        prof_w[0] = clock64() - prof_t0;
+        for (int i = 0; i < 12; ++i) g_prof[blockIdx.x][warp][i] = prof_w[i];
+    }
+#endif
+    // no CTA may leave while a peer can still write its shared memory or arrive on its barriers
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory");
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tb), "n"(512));
+}
+
+// ---- weight builder (plan creation / table updates): a2 + a3 + a4 as 16-bit integers, two 8-bit digits --------------
+// W[m][n] = g[pol, cyl, n] * exp(-2 pi i J[m] n / NP) (eq. (1)+(2) through J), or, with exact
+// pointing, exp(-2 pi i n x[m]) with x = f d sin(theta_m) / c0 turns per feed; row m = [Wr | -Wi] in the
+// K order of prep_tile; value = round(S_c * W) = 65536 d2 + 256 d1 + d0 with balanced digits in [-128, 127].
+constexpr int kWMax = 127 * 65536 + 127 * 256 + 127;   // largest 24-bit weight whose three digits fit in [-128, 127]
+struct WeightParams {
+    uint32_t *wq;
+    int4 *rowsum;
+    const float2 *gains;      // [C][2048] or nullptr (unit)
+    const int32_t *J;         // [C][256]
+    const double *turns;      // [C][256] exact pointing (turns per feed), or nullptr
+    const double *scale;      // [C] S_c
+    int NP;
+};
+
+__global__ void __launch_bounds__(128) build_weights_kernel(const WeightParams wp) {
+    const int set = blockIdx.x;               // ((c * 2 + pol) * 4 + cyl) * 2 + rt
+    const int rt = set & 1, cyl = (set >> 1) & 3, pol = (set >> 3) & 1, c = set >> 4;
+    const int row = threadIdx.x, m = 128 * rt + row, quarter = row >> 5, lane = row & 31;
+    const double S = wp.scale[c];
+    const int J = wp.J[(size_t)c * 256 + m];
+    const double x = wp.turns ? wp.turns[(size_t)c * 256 + m] : 0.0;
+    uint32_t *dst = wp.wq + (size_t)set * kWqWordsPerSet + quarter * (kWCols * 32) + lane;
+    int sum[3] = {0, 0, 0};
+    for (int n4 = 0; n4 < 64; ++n4) {
+        uint32_t w1[3] = {0, 0, 0}, w2[3] = {0, 0, 0};   // digit 2 (top), 1, 0 of the first / second K half
+        for (int b = 0; b < 4; ++b) {
+            const int n = 4 * n4 + b;
+            double sn, cs;
+            if (wp.turns) {
+                double ph = x * (double)n;
+                ph -= rint(ph);
+                sincospi(-2.0 * ph, &sn, &cs);
+            } else {
+                const int k = (J * n) & (wp.NP - 1);
+                sincospi(-2.0 * (double)k / (double)wp.NP, &sn, &cs);
+            }
+            double gr = 1.0, gi = 0.0;
+            if (wp.gains) {
+                const float2 g = wp.gains[(size_t)c * 2048 + (pol * 4 + cyl) * 256 + n];
+                gr = g.x;
+                gi = g.y;
+            }
+            const double wr = gr * cs - gi * sn, wi = gr * sn + gi * cs;
+            const int a[2] = {(int)rint(S * wr), (int)rint(-S * wi)};
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                int v = max(-kWMax, min(kWMax, a[h]));
+                const int d0 = ((v + 128) & 255) - 128;
+                v = (v - d0) >> 8;
+                const int d1 = ((v + 128) & 255) - 128;
+                const int d2 = (v - d1) >> 8;
+                sum[0] += d2;
+                sum[1] += d1;
+                sum[2] += d0;
+                uint32_t *w = h ? w2 : w1;
+                w[0] |= (uint32_t)(d2 & 255) << (8 * b);
+                w[1] |= (uint32_t)(d1 & 255) << (8 * b);
+                w[2] |= (uint32_t)(d0 & 255) << (8 * b);
+            }
+        }
+        // TMEM column of K word kw (bytes 4 kw .. 4 kw + 3) of digit pass p: 128 p + kw; kw = 8 (n4 / 4) + (n4 % 4) [+ 4]
+        const int kw1 = 8 * (n4 >> 2) + (n4 & 3), kw2 = kw1 + 4;
+        auto put = [&](int col, uint32_t v) { dst[(size_t)(col >> 5) * 1024 + (col & 31) * 32] = v; };
+#pragma unroll
+        for (int p = 0; p < 3; ++p) {
+            put(128 * p + kw1, w1[p]);
+            put(128 * p + kw2, w2[p]);
+        }
+    }
+    wp.rowsum[(size_t)set * 128 + row] = make_int4(sum[0], sum[1], sum[2], 0);
+}
+
+}  // namespace chime4
