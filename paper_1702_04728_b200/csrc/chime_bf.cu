@@ -74,6 +74,7 @@ struct chime_bf_plan {
     int32_t *d_J = nullptr;       // [C][256]
     int *d_status = nullptr, *h_status = nullptr;   // mapped host word: which wait timed out (0 = none)
     int max_clusters = 0;         // co-resident clusters of 4 (persistent grid)
+    float *d_scratch = nullptr;   // per-CTA parking space of the tensor-core kernel (32 KiB per CTA)
 };
 
 namespace {
@@ -311,6 +312,7 @@ bool build_tables(chime_bf_plan *pl) {
         cfg.dynamicSmemBytes = chime4::kSmemBytes;
         CUDA_TRY(cudaOccupancyMaxActiveClusters(&pl->max_clusters, chime4::umma_beamform_kernel, &cfg));
         if (pl->max_clusters < 1) { set_err("plan_create: no cluster of 4 CTAs fits on this device"); return false; }
+        CUDA_TRY(cudaMalloc((void **)&pl->d_scratch, (size_t)pl->max_clusters * 4 * chime4::kChunkFrames * 128 * 16 * sizeof(float)));
         CUDA_TRY(cudaHostAlloc((void **)&pl->h_status, 128 * sizeof(int), cudaHostAllocMapped));   // survives a trapped kernel
         memset(pl->h_status, 0, 128 * sizeof(int));
         CUDA_TRY(cudaHostGetDevicePointer((void **)&pl->d_status, pl->h_status, 0));
@@ -439,6 +441,7 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         up.scale = pl->scale;
         up.offset = pl->offset;
         up.status = pl->d_status;
+        up.scratch = pl->d_scratch;
         const long long n_items = (long long)n_chan * ((n_fr + chime4::kChunkFrames - 1) / chime4::kChunkFrames) * 2;
         const int n_cl = (int)std::min<long long>(n_items, pl->max_clusters);
         chime4::umma_beamform_kernel<<<4 * n_cl, chime4::kThreads, chime4::kSmemBytes, st>>>(up);
@@ -870,6 +873,7 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_stage_out);
     cudaFree(pl->d_delay);
     cudaFree(pl->d_peer_out);
+    cudaFree(pl->d_scratch);
     cudaFree(pl->d_wq);
     cudaFree(pl->d_rowsum);
     cudaFree(pl->d_beta);

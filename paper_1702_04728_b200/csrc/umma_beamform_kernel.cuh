@@ -82,6 +82,7 @@ struct Params {
     uint8_t *const *peer_out; // beam-major exchange (chime::beam_major_dst), nullptr = off
     int n_peers, chan_global0;
     float norm, scale, offset;
+    float *scratch;           // [grid][4 frames][4 e][32 beams][16]: polarisation-0 sums parked until pol 1 is done (L2)
     int *status;              // set to non-zero when a wait timed out (the kernel traps afterwards)
 };
 
@@ -106,38 +107,32 @@ __device__ __forceinline__ uint32_t mapa(uint32_t a, uint32_t rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
     return r;
 }
-template <bool CLUSTER>
+// try_wait with a suspend-time hint: the hardware parks the warp until the phase completes (or the hint expires)
+// instead of letting it spin through the issue slots the working warps need.
 __device__ __forceinline__ bool mbar_try(uint32_t a, uint32_t parity) {
     uint32_t ok;
-    if constexpr (CLUSTER)
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
-    else
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(a), "r"(parity), "r"(20000u) : "memory");
     return ok != 0;
 }
-// Waits for the phase of parity `parity` to complete.  A wait that lasts ~2 s is a protocol bug: flag it and trap
-// instead of hanging the GPU.
 #ifdef CHIME_PROF
 __device__ long long g_prof[148 * 4][24][12];
 #define PW(code, stmt) { const long long _t = clock64(); stmt; prof_w[code] += clock64() - _t; }
 #else
 #define PW(code, stmt) { stmt; }
 #endif
-template <bool CLUSTER = false>
+// Waits for the phase of parity `parity` to complete.  A wait of ~2^20 polls (each up to 20 us) is a protocol bug:
+// flag it and trap instead of hanging the GPU.
+__device__ __forceinline__ void mbar_timeout(int *status, int code, uint32_t info) {
+    atomicCAS(status + code * 8 + (blockIdx.x & 7), 0, 1 | ((int)(threadIdx.x >> 5) << 8) | ((int)info << 16));
+    __threadfence_system();
+    for (long long t1 = clock64(); clock64() - t1 < 1500000000ll;) {}
+    __trap();
+}
 __device__ __forceinline__ void mbar_wait(uint32_t a, uint32_t parity, int *status, int code, uint32_t info = 0) {
-    if (mbar_try<CLUSTER>(a, parity)) return;
-    const long long t0 = clock64();
-
-    while (!mbar_try<CLUSTER>(a, parity)) {
-        if (clock64() - t0 > 2000000000ll) {
-            atomicCAS(status + code * 8 + (blockIdx.x & 7), 0, 1 | ((int)(threadIdx.x >> 5) << 8) | ((int)info << 16));
-            __threadfence_system();
-            for (long long t1 = clock64(); clock64() - t1 < 1500000000ll;) {}
-            __trap();
-        }
-    }
+    uint32_t n = 0;
+    while (!mbar_try(a, parity))
+        if (++n > (1u << 20)) mbar_timeout(status, code, info);
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
@@ -267,51 +262,50 @@ __device__ __forceinline__ void tmem_fill16(uint32_t taddr, uint32_t v) {
                  :: "r"(taddr), "r"(v) : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t *v) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                 "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+                 "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                   "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                   "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                 : "r"(taddr) : "memory");
+}
+
+// One digit pass of this thread's 64 columns folded into y; the columns are refilled with the magic constant for the
+// slot's next pass.  Every accumulator column starts from the bit pattern of M = 1.5 * 2^23, so what is loaded is
+// already the float M + a (|a| < 2^22, exact): y = a2 + a1 / 256 + a0 / 65536 in units of the top digit costs one
+// instruction per value and pass.  Column 32 part + j (part 0 = real, 1 = imaginary, j = 16 set + u') goes to
+// y[2 j + part], so that (re, im) pairs and the 16-byte groups the sender stores sit in consecutive registers.
 template <int P>
 __device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64]) {
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
+    for (int c = 0; c < 4; ++c) {   // 16 columns at a time: c = 2 part + set
         uint32_t h[16];
         tmem_ld16(tslot + 16 * c, h);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        tmem_fill16(tslot + 16 * c, kMagicBits);             // ready for the slot's next pass
+        tmem_fill16(tslot + 16 * c, kMagicBits);
+        const int part = c >> 1;
 #pragma unroll
-        for (int i = 0; i < 16; i += 2) {
-            const float2 f = make_float2(__uint_as_float(h[i]), __uint_as_float(h[i + 1]));
-            float2 r;
-            if constexpr (P == 0) r = __fadd2_rn(f, make_float2(-kMagicSum, -kMagicSum));
-            else if constexpr (P == 1) r = __ffma2_rn(f, make_float2(1.0f / 256.0f, 1.0f / 256.0f), make_float2(y[16 * c + i], y[16 * c + i + 1]));
-            else r = __ffma2_rn(f, make_float2(1.0f / 65536.0f, 1.0f / 65536.0f), make_float2(y[16 * c + i], y[16 * c + i + 1]));
-            y[16 * c + i] = r.x;
-            y[16 * c + i + 1] = r.y;
+        for (int i = 0; i < 16; ++i) {
+            const int j = 16 * (c & 1) + i;
+            const float f = __uint_as_float(h[i]);
+            if constexpr (P == 0) y[2 * j + part] = f - kMagicSum;
+            else if constexpr (P == 1) y[2 * j + part] = fmaf(f, 1.0f / 256.0f, y[2 * j + part]);
+            else y[2 * j + part] = fmaf(f, 1.0f / 65536.0f, y[2 * j + part]);
         }
     }
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
-template <int RHO>
-__device__ __forceinline__ void twiddle_fft16(float2 (&a)[16]) {
-    if constexpr (RHO != 0) chime2::time_pretwiddle<RHO, 1>(a);
-    fft_dif<16>(a);
-}
-
-// a: 16 FFT outputs (index i = bin bitrev(i)) of residue `res` -> receive slot of the destination CTA
-// The stores are asynchronous and each one reports its 16 bytes to the destination's mbarrier (complete_tx), so the
-// receiver's wait on that barrier is the only synchronisation: no fence, no arrive on the sending side.
-__device__ __forceinline__ void send16(uint32_t rslot, uint32_t rbar, int cyl, int res, int lane, const float2 (&a)[16]) {
-#pragma unroll
-    for (int ip = 0; ip < 8; ++ip) {
-        const uint32_t addr = rslot + (uint32_t)((((cyl * 2 + res) * 8 + ip) * 32 + lane) * 16);
-        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1,%2,%3,%4}, [%5];"
-                     :: "r"(addr), "f"(a[2 * ip].x), "f"(a[2 * ip].y), "f"(a[2 * ip + 1].x), "f"(a[2 * ip + 1].y), "r"(rbar) : "memory");
-    }
-}
-
-// One tile on the drain side: the three digit passes arrive one after the other in the two rotating accumulator
-// slots (pass 3 tau + p uses slot (tau + p) & 1; n_use counts this group's uses of each slot = the phase of its
-// barriers); each pass is folded into y and the slot handed back at once.
-template <int TT>
-__device__ __forceinline__ void epi_tile(const uint32_t tlane, const uint32_t bar_full0, const uint32_t bar_empty0,
+// One tile on the drain side (the two drain groups take alternate tiles, so that one group's DSMEM stores overlap the
+// other group's drains).  The three digit passes arrive one after the other in the two rotating slots (pass 3 tau + p
+// uses slot (tau + p) & 1; n_use counts this group's uses of each slot = the phase of its barriers); each pass is
+// folded into y and the slot handed back at once.  Odd-residue tiles (tt >= 2) combine E and O' here; the rest of the
+// time transform (twiddle, FFT-16) is linear and runs AFTER the E-W sum on the receiving side.
+// Receive slot layout: [cyl 4][res 2][u' pair 8][beam 32] x {re, im, re, im}.
+__device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, const uint32_t bar_full0, const uint32_t bar_empty0,
                                          uint32_t (&n_use)[2], const uint32_t tau, const uint32_t rslot, const uint32_t rbar,
                                          const int cyl, const int lane, const uint32_t slot_free_bar,
                                          const uint32_t sf_parity, int *status, long long *prof_w) {
@@ -323,40 +317,34 @@ __device__ __forceinline__ void epi_tile(const uint32_t tlane, const uint32_t ba
         ++n_use[slot];
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t tslot = tlane + kWCols + 64 * slot;
-        PW(6, if (p == 0) drain_pass<0>(tslot, y);
+        if (p == 0) drain_pass<0>(tslot, y);
         else if (p == 1) drain_pass<1>(tslot, y);
-        else drain_pass<2>(tslot, y);)
+        else drain_pass<2>(tslot, y);
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty0 + 8 * slot);   // the slot is in registers: hand it back to the issuer
     }
-    float2 a0[16], a1[16];
-#ifdef CHIME_PROF
-    const long long t_fft = clock64();
-#endif
-#pragma unroll
-    for (int u = 0; u < 16; ++u) {
-        a0[u] = make_float2(y[u], y[32 + u]);
-        a1[u] = make_float2(y[16 + u], y[48 + u]);
-    }
-    if constexpr (TT >= 2) {   // A_rho = E + O'/sqrt2, A_{rho+4} = E - O'/sqrt2
+    if (tt >= 2) {   // A_rho = E + O'/sqrt2 (set 0), A_{rho+4} = E - O'/sqrt2 (set 1)
         constexpr float s = 0.70710678118654752440f;
 #pragma unroll
-        for (int u = 0; u < 16; ++u) {
-            const float2 e = a0[u], o = a1[u];
-            a0[u] = __ffma2_rn(o, make_float2(s, s), e);
-            a1[u] = __ffma2_rn(o, make_float2(-s, -s), e);
+        for (int k = 0; k < 32; ++k) {   // k = 2 u' + part
+            const float e = y[k], o = y[32 + k];
+            y[k] = fmaf(s, o, e);
+            y[32 + k] = fmaf(-s, o, e);
         }
     }
-    constexpr int RHO = (TT == 0) ? 0 : (TT == 1) ? 2 : (TT == 2) ? 1 : 3;
-    twiddle_fft16<RHO>(a0);
-    twiddle_fft16<RHO + 4>(a1);
-#ifdef CHIME_PROF
-    prof_w[7] += clock64() - t_fft;
-#endif
     PW(5, mbar_wait(slot_free_bar, sf_parity, status, 5);)     // the destination has consumed this slot's previous tile
-    PW(8, send16(rslot, rbar, cyl, 0, lane, a0);
-    send16(rslot, rbar, cyl, 1, lane, a1);)
+    // Asynchronous stores: each reports its 16 bytes to the destination's mbarrier (complete_tx), so the receiver's
+    // wait on that barrier is the only synchronisation: no fence, no arrive on the sending side.
+#pragma unroll
+    for (int res = 0; res < 2; ++res)
+#pragma unroll
+        for (int ip = 0; ip < 8; ++ip) {
+            const uint32_t addr = rslot + (uint32_t)((((cyl * 2 + res) * 8 + ip) * 32 + lane) * 16);
+            const int k = 32 * res + 4 * ip;
+            asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1,%2,%3,%4}, [%5];"
+                         :: "r"(addr), "f"(y[k]), "f"(y[k + 1]), "f"(y[k + 2]), "f"(y[k + 3]), "r"(rbar) : "memory");
+        }
 }
 
 __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_beamform_kernel(const Params prm) {
@@ -414,11 +402,11 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
         const int nf = min(kChunkFrames, prm.frame0 + prm.n_frames_launch - fr0);          \
         (void)rt; (void)c; (void)fr0; (void)nf;
 
-    // Register budget per warpgroup: 32 / 80 / 120 / 120 / 64 / 64.  setmaxnreg only redistributes what the CTA was
+    // Register budget per warpgroup: 32 / 80 / 112 / 112 / 72 / 72.  setmaxnreg only redistributes what the CTA was
     // launched with (768 x 80), so the six budgets must not add up to more than 6 x 80.
     if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
-    else if (warp >= 16) asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
-    else if (warp >= 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 120;");
+    else if (warp >= 16) asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
+    else if (warp >= 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
 
     if (warp < 2) {
         // ============================== MMA issuers: warp w owns accumulator slot w ==============================
@@ -572,54 +560,50 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
 #pragma unroll 1
                 for (int t = 0; t < ntiles; ++t, ++tau) {
                     if ((int)(tau & 1) != g) continue;
-                    const uint32_t sfp = ((tau >> 1) & 1) ^ 1;
-#ifdef CHIME_PROF
-                    const long long t_tile = clock64();
-#endif
-                    switch (t & 3) {
-                        case 0: epi_tile<0>(tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, sfp, status, prof_w); break;
-                        case 1: epi_tile<1>(tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, sfp, status, prof_w); break;
-                        case 2: epi_tile<2>(tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, sfp, status, prof_w); break;
-                        default: epi_tile<3>(tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, sfp, status, prof_w); break;
-                    }
-#ifdef CHIME_PROF
-                    prof_w[10] += clock64() - t_tile;
-#endif
+                    epi_tile(t & 3, tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, ((tau >> 1) & 1) ^ 1, status, prof_w);
                 }
             }
         }
     } else {
-        // ============================== receive side: E-W, detect, integrate, output ==============================
-        const int ip = warp - 16, rtid = tid - 512;
+        // ============================== receive side: E-W, time FFT-16, detect, integrate, output ==============================
+        // Two phases per tile over the slot [cyl][res][u' pair][beam] x {re, im, re, im}:
+        //   1. thread <-> (beam = lane, u' pair = warp): Horner in beta_e over the 4 cylinders for both residues, the 4
+        //      E-W beams written back IN PLACE (cell index cyl -> e);
+        //   2. thread <-> (beam, residue = warp & 1, E-W beam = warp >> 1): 16 values of u', twiddle W_128^{rho u'},
+        //      FFT-16, |.|^2 into the 16 fine channels of the current frame.
+        // Per frame the two residue halves meet in shared memory and the odd warps, which then hold all 16 fine channels
+        // of (E-W beam, beam), park the polarisation-0 sums in a per-CTA scratch (L2) and finish the frame after pol 1.
+        const int rw = warp - 16;
+        const int res2 = rw & 1, e2 = rw >> 1;
         uint32_t sf_remote[4][2];
 #pragma unroll
         for (int s = 0; s < 4; ++s) {
             sf_remote[s][0] = mapa(BAR(B_SLOT_FREE + 2 * rank + 0), s);
             sf_remote[s][1] = mapa(BAR(B_SLOT_FREE + 2 * rank + 1), s);
         }
-        float *ost = reinterpret_cast<float *>(smem + kOfsOut);
-        const int g0 = (bitrev(2 * ip, 4) + 8) & 15, g1 = (bitrev(2 * ip + 1, 4) + 8) & 15;
+        float *ost = reinterpret_cast<float *>(smem + kOfsOut) + (e2 * 32 + lane) * 17;
+        float4 *scr = reinterpret_cast<float4 *>(prm.scratch + ((size_t)blockIdx.x * kChunkFrames * 128 + e2 * 32 + lane) * 16);
         uint32_t tau = 0;
         ITEM_LOOP
             float2 be[4];
 #pragma unroll
             for (int e = 0; e < 4; ++e) be[e] = __ldg(prm.beta + (size_t)c * 4 + e);
-            float acc[kChunkFrames][4][2];
-#pragma unroll
-            for (int f = 0; f < kChunkFrames; ++f)
-#pragma unroll
-                for (int e = 0; e < 4; ++e) acc[f][e][0] = acc[f][e][1] = 0.f;
+            const float nrm = prm.norm * __ldg(prm.inv_s2 + c);
 #pragma unroll 1
             for (int pol = 0; pol < 2; ++pol) {
-#pragma unroll
-                for (int fr = 0; fr < kChunkFrames; ++fr) {
-                    if (fr < nf) {
 #pragma unroll 1
-                        for (int t = 0; t < 12; ++t, ++tau) {
-                            const uint32_t s = tau & 1;
-                            PW(10, mbar_wait(BAR(B_RECV_FULL + s), (tau >> 1) & 1, status, 10, tau);)
-                            if (ip == 0 && lane == 0) mbar_expect_tx(BAR(B_RECV_FULL + s), kRecvBytes);   // arm the slot's next tile
-                            const unsigned char *base = smem + kOfsRecv + s * kRecvBytes + (ip * 32 + lane) * 16;
+                for (int fr = 0; fr < nf; ++fr) {
+                    float acc[16];
+#pragma unroll
+                    for (int g = 0; g < 16; ++g) acc[g] = 0.f;
+#pragma unroll 1
+                    for (int t = 0; t < 12; ++t, ++tau) {
+                        const uint32_t s = tau & 1;
+                        PW(10, mbar_wait(BAR(B_RECV_FULL + s), (tau >> 1) & 1, status, 10, tau);)
+                        if (rw == 0 && lane == 0) mbar_expect_tx(BAR(B_RECV_FULL + s), kRecvBytes);   // arm the slot's next tile
+                        unsigned char *slot = smem + kOfsRecv + s * kRecvBytes + lane * 16;
+                        {   // ---- phase 1: (beam, u' pair = rw), both residues
+                            unsigned char *base = slot + rw * 512;
 #pragma unroll
                             for (int res = 0; res < 2; ++res) {
                                 float4 sv[4];
@@ -638,56 +622,83 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                                         za = __ffma2_rn(make_float2(za.y, za.x), by, ta);
                                         zb = __ffma2_rn(make_float2(zb.y, zb.x), by, tb2);
                                     }
-                                    acc[fr][e][0] = fmaf(za.x, za.x, fmaf(za.y, za.y, acc[fr][e][0]));
-                                    acc[fr][e][1] = fmaf(zb.x, zb.x, fmaf(zb.y, zb.y, acc[fr][e][1]));
+                                    *reinterpret_cast<float4 *>(base + ((e * 2 + res) * 8) * 512) = make_float4(za.x, za.y, zb.x, zb.y);
                                 }
-                            }
-                            __syncwarp();
-                            if (lane == 0) {
-#pragma unroll
-                                for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc][s]);
                             }
                         }
+                        bar_sync_named(1, 256);
+                        {   // ---- phase 2: (beam, residue = res2, E-W beam = e2)
+                            const unsigned char *base = slot + ((e2 * 2 + res2) * 8) * 512;
+                            float2 a[16];
+#pragma unroll
+                            for (int k = 0; k < 8; ++k) {
+                                const float4 v = *reinterpret_cast<const float4 *>(base + k * 512);
+                                a[2 * k] = make_float2(v.x, v.y);
+                                a[2 * k + 1] = make_float2(v.z, v.w);
+                            }
+                            // residue of (tile type, column set): {0,4}, {2,6}, {1,5}, {3,7}
+                            const int tt = t & 3;
+                            const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
+#pragma unroll
+                            for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], chime2::c_tw128[(rho * u) & 127]);
+                            fft_dif<16>(a);
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) {
+                                const int g = (bitrev(i, 4) + 8) & 15;
+                                acc[g] = fmaf(a[i].x, a[i].x, fmaf(a[i].y, a[i].y, acc[g]));
+                            }
+                        }
+                        __syncwarp();
+                        if (lane == 0) {
+#pragma unroll
+                            for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc][s]);
+                        }
                     }
-                }
-            }
-            // ---- item epilogue: a9 normalise, a10 quantise, one 16-byte store per beam ----
-            const float nrm = prm.norm * __ldg(prm.inv_s2 + c);
+                    // ---- frame end: a9 sum of the two residue halves (+ pol 0), normalise, a10 quantise, 16-byte store per beam
+                    if (res2 == 0) {
 #pragma unroll
-            for (int fr = 0; fr < kChunkFrames; ++fr) {
-                if (fr < nf) {
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        ost[(e * 32 + lane) * 17 + g0] = acc[fr][e][0] * nrm;
-                        ost[(e * 32 + lane) * 17 + g1] = acc[fr][e][1] * nrm;
+                        for (int g = 0; g < 16; ++g) ost[g] = acc[g];
                     }
                     bar_sync_named(1, 256);
-                    if (rtid < 128) {
-                        const int e = rtid >> 5, ns = 128 * rt + 32 * (int)rank + (rtid & 31);
-                        const int Rf = fr0 + fr;
-                        const float *v = ost + rtid * 17;
-                        const size_t ob = ((((size_t)c * prm.n_frames + Rf) * 4 + e) * 256 + ns) * 16;
-                        if (prm.out_f32 != nullptr) {
-                            float4 *dst = reinterpret_cast<float4 *>(prm.out_f32 + ob);
+                    if (res2 == 1) {
 #pragma unroll
-                            for (int k = 0; k < 4; ++k) dst[k] = make_float4(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
+                        for (int g = 0; g < 16; ++g) acc[g] += ost[g];
+                        if (pol == 0) {
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) scr[fr * 128 * 4 + k] = make_float4(acc[4 * k], acc[4 * k + 1], acc[4 * k + 2], acc[4 * k + 3]);
                         } else {
-                            uint32_t qw[4];
 #pragma unroll
                             for (int k = 0; k < 4; ++k) {
-                                uint32_t word = 0;
-#pragma unroll
-                                for (int b = 0; b < 4; ++b) {
-                                    const float x = fmaf(v[4 * k + b], prm.scale, prm.offset);
-                                    word |= (uint32_t)__float2int_rn(fminf(fmaxf(x, 0.f), 255.f)) << (8 * b);
-                                }
-                                qw[k] = word;
+                                const float4 v = scr[fr * 128 * 4 + k];
+                                acc[4 * k] = (acc[4 * k] + v.x) * nrm;
+                                acc[4 * k + 1] = (acc[4 * k + 1] + v.y) * nrm;
+                                acc[4 * k + 2] = (acc[4 * k + 2] + v.z) * nrm;
+                                acc[4 * k + 3] = (acc[4 * k + 3] + v.w) * nrm;
                             }
-                            const uint4 qv = make_uint4(qw[0], qw[1], qw[2], qw[3]);
-                            if (prm.peer_out != nullptr)
-                                *chime::beam_major_dst(prm.peer_out, prm.n_peers, prm.chan_global0 + c, prm.n_frames, Rf, e * 256 + ns) = qv;
-                            else
-                                *reinterpret_cast<uint4 *>(prm.out_u8 + ob) = qv;
+                            const int ns = 128 * rt + 32 * (int)rank + lane, Rf = fr0 + fr;
+                            const size_t ob = ((((size_t)c * prm.n_frames + Rf) * 4 + e2) * 256 + ns) * 16;
+                            if (prm.out_f32 != nullptr) {
+                                float4 *dst = reinterpret_cast<float4 *>(prm.out_f32 + ob);
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) dst[k] = make_float4(acc[4 * k], acc[4 * k + 1], acc[4 * k + 2], acc[4 * k + 3]);
+                            } else {
+                                uint32_t qw[4];
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) {
+                                    uint32_t word = 0;
+#pragma unroll
+                                    for (int b = 0; b < 4; ++b) {
+                                        const float x = fmaf(acc[4 * k + b], prm.scale, prm.offset);
+                                        word |= (uint32_t)__float2int_rn(fminf(fmaxf(x, 0.f), 255.f)) << (8 * b);
+                                    }
+                                    qw[k] = word;
+                                }
+                                const uint4 qv = make_uint4(qw[0], qw[1], qw[2], qw[3]);
+                                if (prm.peer_out != nullptr)
+                                    *chime::beam_major_dst(prm.peer_out, prm.n_peers, prm.chan_global0 + c, prm.n_frames, Rf, e2 * 256 + ns) = qv;
+                                else
+                                    *reinterpret_cast<uint4 *>(prm.out_u8 + ob) = qv;
+                            }
                         }
                     }
                     bar_sync_named(1, 256);
