@@ -583,7 +583,7 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
         const char *kv = getenv("CHIME_BF_KERNEL");   // A/B switch: v1 generic, v2 block-synchronous mma, v3 warp-specialised (default)
         pl->use_ws = !kv || !strcmp(kv, "v3") || !strcmp(kv, "v4");
     }
-    pl->use_umma = p.upchan_len == 128 && getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v4");   // development switch, goes when v4 wins
+    pl->use_umma = p.upchan_len == 128 && !(getenv("CHIME_BF_KERNEL") && strcmp(getenv("CHIME_BF_KERNEL"), "v4"));   // development switch, to be removed
     pl->n_pass = (p.zero_pad == 1024 && p.upchan_len == 128 && pl->use_ws && !pl->use_umma) ? 2 : 1;
     pl->use_mma = ((p.zero_pad == 512 || p.zero_pad == 256 || pl->n_pass == 2) && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1")) && !pl->use_umma;
     cudaGetDevice(&pl->device);

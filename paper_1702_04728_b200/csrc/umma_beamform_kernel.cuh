@@ -306,15 +306,17 @@ __device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64])
 // time transform (twiddle, FFT-16) is linear and runs AFTER the E-W sum on the receiving side.
 // Receive slot layout: [cyl 4][res 2][u' pair 8][beam 32] x {re, im, re, im}.
 __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, const uint32_t bar_full0, const uint32_t bar_empty0,
-                                         uint32_t (&n_use)[2], const uint32_t tau, const uint32_t rslot, const uint32_t rbar,
+                                         uint32_t &n_use0, uint32_t &n_use1, const uint32_t tau, const uint32_t rslot, const uint32_t rbar,
                                          const int cyl, const int lane, const uint32_t slot_free_bar,
                                          const uint32_t sf_parity, int *status, long long *prof_w) {
     float y[64];
 #pragma unroll
     for (int p = 0; p < 3; ++p) {
         const uint32_t slot = (tau + p) & 1;     // = (3 tau + p) & 1
-        PW(9, mbar_wait(bar_full0 + 8 * slot, n_use[slot] & 1, status, 9, tau);)
-        ++n_use[slot];
+        const uint32_t use = slot ? n_use1 : n_use0;
+        PW(9, mbar_wait(bar_full0 + 8 * slot, use & 1, status, 9, tau);)
+        n_use0 += 1 - slot;
+        n_use1 += slot;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t tslot = tlane + kWCols + 64 * slot;
         if (p == 0) drain_pass<0>(tslot, y);
@@ -418,8 +420,8 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
         // order; the issuer waits for the drain of the slot's PREVIOUS use, whichever group that was.
         const uint32_t myslot = warp;
         uint32_t tau = 0, seg = 0;
-        uint32_t n_use[2] = {1, 0};     // drains of my slot requested so far, per group (group 0's initial fill counts)
-        int prev_g = 0;                 // group that drains (fills) my slot before my next pass
+        uint32_t n_use0 = 1, n_use1 = 0;   // drains of my slot requested so far, per group (group 0's initial fill counts)
+        int prev_g = 0;                    // group that drains (fills) my slot before my next pass
         ITEM_LOOP
             for (int pol = 0; pol < 2; ++pol) {
                 PW(1, mbar_wait(BAR(B_W_READY), seg & 1, status, 1, seg);)
@@ -434,7 +436,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                         const uint32_t pi = 3 * tau + p;
                         if ((pi & 1) != myslot) continue;
                         const int g = tau & 1;
-                        PW(3, mbar_wait(BAR(B_ACC_EMPTY + 2 * prev_g + myslot), (n_use[prev_g] - 1) & 1, status, 3, tau);)
+                        PW(3, mbar_wait(BAR(B_ACC_EMPTY + 2 * prev_g + myslot), ((prev_g ? n_use1 : n_use0) - 1) & 1, status, 3, tau);)
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         if (elect_one()) {
                             const uint32_t d = tb + kWCols + 64 * myslot;
@@ -450,7 +452,8 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                             umma_commit(BAR(B_ACC_FULL + 2 * g + myslot));
                         }
                         __syncwarp();
-                        ++n_use[g];
+                        n_use0 += 1 - g;
+                        n_use1 += g;
                         prev_g = g;
                     }
                     if (elect_one()) umma_commit(BAR(B_BOP_EMPTY + s));   // both issuers: the B tile is free when all 3 passes are done
@@ -541,7 +544,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
         const uint32_t rfull = mapa(BAR(B_RECV_FULL + g), q);
         const uint32_t sfree = BAR(B_SLOT_FREE + 2 * q + g);
         const uint32_t accf = BAR(B_ACC_FULL + 2 * g), acce = BAR(B_ACC_EMPTY + 2 * g);
-        uint32_t n_use[2] = {0, 0};
+        uint32_t n_use0 = 0, n_use1 = 0;
         uint32_t tau = 0;
         if (g == 0) {   // both accumulator slots start from the magic constant: group 0's "drain number 0" of each slot
 #pragma unroll
@@ -560,7 +563,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
 #pragma unroll 1
                 for (int t = 0; t < ntiles; ++t, ++tau) {
                     if ((int)(tau & 1) != g) continue;
-                    epi_tile(t & 3, tlane, accf, acce, n_use, tau, rslot, rfull, rank, lane, sfree, ((tau >> 1) & 1) ^ 1, status, prof_w);
+                    epi_tile(t & 3, tlane, accf, acce, n_use0, n_use1, tau, rslot, rfull, rank, lane, sfree, ((tau >> 1) & 1) ^ 1, status, prof_w);
                 }
             }
         }
@@ -575,12 +578,9 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
         // of (E-W beam, beam), park the polarisation-0 sums in a per-CTA scratch (L2) and finish the frame after pol 1.
         const int rw = warp - 16;
         const int res2 = rw & 1, e2 = rw >> 1;
-        uint32_t sf_remote[4][2];
+        uint32_t sf_remote[4];   // slot 0's barrier of this CTA's beams in each source CTA; slot 1's is 8 bytes further
 #pragma unroll
-        for (int s = 0; s < 4; ++s) {
-            sf_remote[s][0] = mapa(BAR(B_SLOT_FREE + 2 * rank + 0), s);
-            sf_remote[s][1] = mapa(BAR(B_SLOT_FREE + 2 * rank + 1), s);
-        }
+        for (int s = 0; s < 4; ++s) sf_remote[s] = mapa(BAR(B_SLOT_FREE + 2 * rank), s);
         float *ost = reinterpret_cast<float *>(smem + kOfsOut) + (e2 * 32 + lane) * 17;
         float4 *scr = reinterpret_cast<float4 *>(prm.scratch + ((size_t)blockIdx.x * kChunkFrames * 128 + e2 * 32 + lane) * 16);
         uint32_t tau = 0;
@@ -651,7 +651,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                         __syncwarp();
                         if (lane == 0) {
 #pragma unroll
-                            for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc][s]);
+                            for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc] + 8 * s);
                         }
                     }
                     // ---- frame end: a9 sum of the two residue halves (+ pol 0), normalise, a10 quantise, 16-byte store per beam
