@@ -342,17 +342,4 @@ beamform_fused_kernel(const KernelParams prm) {
     }
 }
 
-// Step a1 alone (bit-exact check of the decode): byte -> (re, im) int8.
-__global__ void unpack_kernel(const uint8_t *__restrict__ in, size_t n, int8_t *__restrict__ out) {
-    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (; i < n; i += stride) {
-        const uint32_t b = in[i];
-        char2 v;
-        v.x = (signed char)((int)(b >> 4) - 8);
-        v.y = (signed char)((int)(b & 15u) - 8);
-        reinterpret_cast<char2 *>(out)[i] = v;
-    }
-}
-
 }  // namespace chime

@@ -13,8 +13,6 @@
 #include <vector>
 
 #include "beamform_kernel.cuh"
-#include "beamform_mma_kernel.cuh"
-#include "beamform_ws_kernel.cuh"
 #include "dedisperse_kernel.cuh"
 #include "umma_beamform_kernel.cuh"
 
@@ -50,10 +48,6 @@ struct chime_bf_plan {
     int16_t *d_slot_of_m = nullptr;
     float2 *d_tw_np = nullptr;
     float2 *d_tw_u = nullptr;
-    uint2 *d_bfrag = nullptr;  // tensor-core B fragments of the folded weights (zero_pad 512, upchan 128 path)
-    bool use_mma = false;
-    bool use_ws = false;       // warp-specialised variant of the tensor-core path (default)
-    int n_pass = 1;            // zero_pad 1024 on the tensor-core kernel: two passes (even / odd bins), see build_index_tables
     // staging for execute_host
     uint8_t *d_stage_in = nullptr;
     uint8_t *d_stage_out = nullptr;
@@ -108,6 +102,12 @@ int32_t ns_bin_sintheta(int NP, double f_mhz, double d_m, double s) {
     return (int32_t)j;
 }
 
+bool gains_finite(const float *g, size_t n) {
+    for (size_t i = 0; i < n; ++i)
+        if (!std::isfinite(g[i])) return false;
+    return true;
+}
+
 template <typename T>
 bool upload(T **dst, const std::vector<T> &src) {
     CUDA_TRY(cudaMalloc((void **)dst, src.size() * sizeof(T)));
@@ -142,36 +142,6 @@ bool build_index_tables(chime_bf_plan *pl, cudaStream_t st) {
             if (sl[j] == 0) sl[j] = ns++;
         for (int m = 0; m < 256; ++m) slot_of_m[(size_t)c * 256 + m] = sl[J[m]];
     }
-    if (pl->use_mma && NP == 1024) {
-        // zero_pad 1024 as TWO passes of the 512-point kernel: X[j] = sum_n v[n] W_1024^{n j}.
-        //   pass 0, j even:  bin j/2 of the 512-point transform of v[n]
-        //   pass 1, j odd:   bin (j-1)/2 of the 512-point transform of v[n] W_1024^n  (the factor is folded into
-        //                    the pass's E-W weights, build_weight_tables)
-        // Every beam has one bin, hence one pass; the other pass's slot_of_m is -1 and its epilogue skips the beam.
-        std::vector<int16_t> s2((size_t)2 * C * 512, (int16_t)-1), m2((size_t)2 * C * 256, (int16_t)-1);
-        for (int pass = 0; pass < 2; ++pass)
-            for (int c = 0; c < C; ++c) {
-                int16_t *sl = &s2[((size_t)pass * C + c) * 512];
-                const int32_t *J = &pl->J[(size_t)c * 256];
-                for (int m = 0; m < 256; ++m)
-                    if ((J[m] & 1) == pass) sl[J[m] >> 1] = 0;
-                int16_t ns = 0;
-                for (int j = 0; j < 512; ++j)
-                    if (sl[j] == 0) sl[j] = ns++;
-                for (int m = 0; m < 256; ++m)
-                    if ((J[m] & 1) == pass) m2[((size_t)pass * C + c) * 256 + m] = sl[J[m] >> 1];
-            }
-        slot.swap(s2);
-        slot_of_m.swap(m2);
-    }
-    if (pl->use_mma && NP == 256) {
-        // zero_pad 256 on the tensor-core kernels: bin j of the 256-point transform IS bin 2 j of the 512-point
-        // zero-padded one, so the kernel runs unchanged on a 512-entry map whose odd bins are unused.
-        std::vector<int16_t> slot512((size_t)C * 512, (int16_t)-1);
-        for (int c = 0; c < C; ++c)
-            for (int j = 0; j < 256; ++j) slot512[(size_t)c * 512 + 2 * j] = slot[(size_t)c * 256 + j];
-        slot.swap(slot512);
-    }
     return upload_on(&pl->d_slot, slot, st) && upload_on(&pl->d_slot_of_m, slot_of_m, st);
 }
 
@@ -203,44 +173,6 @@ bool build_weight_tables(chime_bf_plan *pl, cudaStream_t st) {
             }
         }
     }
-    // Tensor-core path (beamform_mma_kernel.cuh): per (c, pol, beam pair ep, feed n) the 8 x 8 real
-    // embedding of the 4 cyl x 2 beam complex weights, as mma.m16n8k8 B fragments (lane = 4 g + tq holds
-    // rows k = 2 tq, 2 tq + 1 of column g), scaled by 2^9 and split hi + lo in fp16.  Columns 4..7 are
-    // zero, so only lanes 0..15 are stored.
-    std::vector<uint2> bfrag;
-    if (pl->use_mma) {
-        const size_t per_pass = (size_t)C * 2 * 2 * 256 * 16;
-        bfrag.resize(per_pass * pl->n_pass);
-        auto split = [](float v, uint16_t &hi, uint16_t &lo) {
-            const __half h = __float2half_rn(v);
-            const __half l = __float2half_rn(v - __half2float(h));
-            memcpy(&hi, &h, 2);
-            memcpy(&lo, &l, 2);
-        };
-        for (int pass = 0; pass < pl->n_pass; ++pass)
-        for (int c = 0; c < C; ++c)
-            for (int pol = 0; pol < 2; ++pol)
-                for (int ep = 0; ep < 2; ++ep)
-                    for (int n = 0; n < 256; ++n)
-                        for (int lane = 0; lane < 16; ++lane) {
-                            const int g = lane >> 2, cyl = lane & 3, e = 2 * ep + (g >> 1), ro = g & 1;
-                            float2 w = wp[((((size_t)c * 2 + pol) * 4 + e) * 4 + cyl) * 256 + n];
-                            if (pass == 1) {   // odd bins of the 1024-point transform: v[n] W_1024^n (double, then float)
-                                const double a = -2.0 * kPi * (double)n / 1024.0, cr = std::cos(a), ci = std::sin(a);
-                                w = make_float2((float)((double)w.x * cr - (double)w.y * ci),
-                                                (float)((double)w.x * ci + (double)w.y * cr));
-                            }
-                            // output re: k=(cyl,re)-> wr, k=(cyl,im)-> -wi ; output im: wi, wr
-                            const float k0 = 512.0f * (ro == 0 ? w.x : w.y);
-                            const float k1 = 512.0f * (ro == 0 ? -w.y : w.x);
-                            uint16_t h0, l0, h1, l1;
-                            split(k0, h0, l0);
-                            split(k1, h1, l1);
-                            bfrag[pass * per_pass + ((((size_t)c * 2 + pol) * 2 + ep) * 256 + n) * 16 + lane] =
-                                make_uint2((uint32_t)h0 | ((uint32_t)h1 << 16), (uint32_t)l0 | ((uint32_t)l1 << 16));
-                        }
-    }
-    if (pl->use_mma && !upload_on(&pl->d_bfrag, bfrag, st)) return false;
     return upload_on(&pl->d_wp, wp, st);
 }
 
@@ -296,7 +228,7 @@ bool build_umma_weights(chime_bf_plan *pl, cudaStream_t st) {
 }
 
 bool build_tables(chime_bf_plan *pl) {
-    const int NP = pl->use_mma ? 512 : pl->NP, U = pl->U;   // the tensor-core kernels always transform 512 points
+    const int NP = pl->NP, U = pl->U;
     if (!build_index_tables(pl, nullptr)) return false;
     if (pl->use_umma) {
         std::vector<float2> tw128(128);
@@ -304,7 +236,7 @@ bool build_tables(chime_bf_plan *pl) {
             const double a = -2.0 * kPi * (double)k / 128.0;
             tw128[k] = make_float2((float)std::cos(a), (float)std::sin(a));
         }
-        CUDA_TRY(cudaMemcpyToSymbol(chime2::c_tw128, tw128.data(), sizeof(float2) * 128));
+        CUDA_TRY(cudaMemcpyToSymbol(chime4::c_tw128, tw128.data(), sizeof(float2) * 128));
         CUDA_TRY(cudaFuncSetAttribute(chime4::umma_beamform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, chime4::kSmemBytes));
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(4 * 148);
@@ -312,7 +244,7 @@ bool build_tables(chime_bf_plan *pl) {
         cfg.dynamicSmemBytes = chime4::kSmemBytes;
         CUDA_TRY(cudaOccupancyMaxActiveClusters(&pl->max_clusters, chime4::umma_beamform_kernel, &cfg));
         if (pl->max_clusters < 1) { set_err("plan_create: no cluster of 4 CTAs fits on this device"); return false; }
-        CUDA_TRY(cudaMalloc((void **)&pl->d_scratch, (size_t)pl->max_clusters * 4 * chime4::kChunkFrames * 128 * 16 * sizeof(float)));
+        CUDA_TRY(cudaMalloc((void **)&pl->d_scratch, (size_t)pl->max_clusters * 4 * chime4::kMaxChunkFrames * 128 * 16 * sizeof(float)));
         CUDA_TRY(cudaHostAlloc((void **)&pl->h_status, 128 * sizeof(int), cudaHostAllocMapped));   // survives a trapped kernel
         memset(pl->h_status, 0, 128 * sizeof(int));
         CUDA_TRY(cudaHostGetDevicePointer((void **)&pl->d_status, pl->h_status, 0));
@@ -329,20 +261,6 @@ bool build_tables(chime_bf_plan *pl) {
     for (int k = 0; k < U; ++k) {
         const double a = -2.0 * kPi * (double)k / (double)U;
         tw_u[k] = make_float2((float)std::cos(a), (float)std::sin(a));
-    }
-    if (pl->use_mma) {
-        std::vector<float2> tw128(128);
-        for (int k = 0; k < 128; ++k) {
-            const double a = -2.0 * kPi * (double)k / 128.0;
-            tw128[k] = make_float2((float)std::cos(a), (float)std::sin(a));
-        }
-        CUDA_TRY(cudaMemcpyToSymbol(chime2::c_tw128, tw128.data(), sizeof(float2) * 128));
-        CUDA_TRY(cudaFuncSetAttribute(chime2::beamform_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      chime2::kSmemBytes));
-        CUDA_TRY(cudaFuncSetAttribute(chime3::beamform_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      chime3::kSmemBytesWs));
-        CUDA_TRY(cudaFuncSetAttribute(chime3::beamform_ws_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      chime3::kSmemBytesWs));
     }
     CUDA_TRY(cudaMalloc((void **)&pl->d_delay, (size_t)pl->C * 16 * sizeof(int32_t)));
     CUDA_TRY(cudaMalloc((void **)&pl->d_peer_out, 64 * sizeof(uint8_t *)));
@@ -442,50 +360,17 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         up.offset = pl->offset;
         up.status = pl->d_status;
         up.scratch = pl->d_scratch;
-        const long long n_items = (long long)n_chan * ((n_fr + chime4::kChunkFrames - 1) / chime4::kChunkFrames) * 2;
+        // frames per work item: as many as possible (the weights are reloaded twice per item), while the launch still
+        // has at least 8 items per cluster to balance the persistent grid
+        int chunk = chime4::kMaxChunkFrames;
+        while (chunk > 1 && (long long)n_chan * ((n_fr + chunk - 1) / chunk) * 2 < 8LL * pl->max_clusters) chunk >>= 1;
+        up.chunk_frames = chunk;
+        const long long n_items = (long long)n_chan * ((n_fr + chunk - 1) / chunk) * 2;
         const int n_cl = (int)std::min<long long>(n_items, pl->max_clusters);
         chime4::umma_beamform_kernel<<<4 * n_cl, chime4::kThreads, chime4::kSmemBytes, st>>>(up);
         const cudaError_t e4 = cudaGetLastError();
         if (e4 != cudaSuccess) {
             set_err("kernel launch failed: %s", cudaGetErrorString(e4));
-            return CHIME_BF_E_CUDA;
-        }
-        return CHIME_BF_OK;
-    }
-    if (pl->use_mma) {
-        chime2::Params mp;
-        mp.in = in;
-        mp.out_u8 = out_u8;
-        mp.out_f32 = out_f32;
-        mp.bfrag = pl->d_bfrag;
-        mp.slot = pl->d_slot;
-        mp.slot_of_m = pl->d_slot_of_m;
-        mp.tw_np = pl->d_tw_np;
-        mp.n_time = pl->T;
-        mp.n_frames = pl->R;
-        mp.chan0 = chan0;
-        mp.frame0 = frame0;
-        mp.n_frames_launch = n_fr;
-        mp.peer_out = peer_out;
-        mp.n_peers = n_peers;
-        mp.chan_global0 = chan_global0;
-        mp.norm = pl->norm;
-        mp.qscale = pl->norm * pl->scale;
-        mp.qoffset = pl->offset;
-        for (int pass = 0; pass < pl->n_pass; ++pass) {
-            mp.bfrag = pl->d_bfrag + (size_t)pass * pl->C * 2 * 2 * 256 * 16;
-            mp.slot = pl->d_slot + (size_t)pass * pl->C * 512;
-            mp.slot_of_m = pl->d_slot_of_m + (size_t)pass * pl->C * 256;
-            if (pl->use_ws && pl->NP == 256)
-                chime3::beamform_ws_kernel<true><<<n_chan * n_fr * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
-            else if (pl->use_ws)
-                chime3::beamform_ws_kernel<false><<<n_chan * n_fr * 2, chime2::kThreads, chime3::kSmemBytesWs, st>>>(mp);
-            else
-                chime2::beamform_mma_kernel<<<n_chan * n_fr * 2, chime2::kThreads, chime2::kSmemBytes, st>>>(mp);
-        }
-        const cudaError_t e2 = cudaGetLastError();
-        if (e2 != cudaSuccess) {
-            set_err("kernel launch failed: %s", cudaGetErrorString(e2));
             return CHIME_BF_E_CUDA;
         }
         return CHIME_BF_OK;
@@ -579,20 +464,21 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     pl->scale = p.scale > 0.f ? p.scale : 1.0f / 64.0f;
     pl->offset = p.scale > 0.f ? p.offset : 128.0f;
     pl->norm = (float)(1.0 / (256.0 * 4.0 * (double)p.upchan_len));
-    {
-        const char *kv = getenv("CHIME_BF_KERNEL");   // A/B switch: v1 generic, v2 block-synchronous mma, v3 warp-specialised (default)
-        pl->use_ws = !kv || !strcmp(kv, "v3") || !strcmp(kv, "v4");
-    }
-    pl->use_umma = p.upchan_len == 128 && !(getenv("CHIME_BF_KERNEL") && strcmp(getenv("CHIME_BF_KERNEL"), "v4"));   // development switch, to be removed
-    pl->n_pass = (p.zero_pad == 1024 && p.upchan_len == 128 && pl->use_ws && !pl->use_umma) ? 2 : 1;
-    pl->use_mma = ((p.zero_pad == 512 || p.zero_pad == 256 || pl->n_pass == 2) && p.upchan_len == 128) && !(getenv("CHIME_BF_KERNEL") && !strcmp(getenv("CHIME_BF_KERNEL"), "v1")) && !pl->use_umma;
+    pl->use_umma = p.upchan_len == 128;   // upchan 256 runs the fp32 kernel of beamform_kernel.cuh
     cudaGetDevice(&pl->device);
     pl->fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
     pl->d_feed = p.feed_spacing_m > 0 ? p.feed_spacing_m : 0.3048;
     pl->d_cyl = p.cyl_spacing_m > 0 ? p.cyl_spacing_m : 22.0;
     pl->freq.resize(p.n_coarse);
     for (int c = 0; c < p.n_coarse; ++c) pl->freq[c] = p.freq_mhz ? p.freq_mhz[c] : 800.0 - (double)c * 0.390625;
-    if (p.gains) pl->gains.assign(p.gains, p.gains + (size_t)p.n_coarse * 2048 * 2);
+    if (p.gains) {
+        if (!gains_finite(p.gains, (size_t)p.n_coarse * 2048 * 2)) {
+            set_err("plan_create: gains must be finite");
+            delete pl;
+            return nullptr;
+        }
+        pl->gains.assign(p.gains, p.gains + (size_t)p.n_coarse * 2048 * 2);
+    }
     if (p.ns_sin_theta) pl->ns_sin.assign(p.ns_sin_theta, p.ns_sin_theta + 256);
     for (int e = 0; e < 4; ++e) pl->ew_deg[e] = p.ew_angles_deg[e];
     bool ok = build_tables(pl);
@@ -638,10 +524,6 @@ int chime_bf_execute_beam_major(chime_bf_plan *pl, void *stream, const uint8_t *
             set_err("execute_beam_major: peer buffer %d is null or not 16-byte aligned", d);
             return CHIME_BF_E_ALIGNMENT;
         }
-    if (pl->use_mma && !pl->use_ws) {
-        set_err("execute_beam_major: not available with CHIME_BF_KERNEL=v2");
-        return CHIME_BF_E_UNSUPPORTED;
-    }
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e = cudaMemcpyAsync(pl->d_peer_out, peer_out, n_peers * sizeof(uint8_t *), cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) { set_err("execute_beam_major: %s", cudaGetErrorString(e)); return CHIME_BF_E_CUDA; }
@@ -722,6 +604,7 @@ int chime_bf_execute_host(chime_bf_plan *pl, void *stream, const uint8_t *in_hos
 
 int chime_bf_update_gains(chime_bf_plan *pl, void *stream, const float *gains) {
     if (!pl) { set_err("update_gains: null plan"); return CHIME_BF_E_INVALID_ARG; }
+    if (gains && !gains_finite(gains, (size_t)pl->C * 2048 * 2)) { set_err("update_gains: gains must be finite"); return CHIME_BF_E_INVALID_ARG; }
     if (gains) pl->gains.assign(gains, gains + (size_t)pl->C * 2048 * 2);
     else pl->gains.clear();
     if (pl->use_umma) return build_umma_weights(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
@@ -835,7 +718,7 @@ int chime_bf_debug_unpack(chime_bf_plan *plan, void *stream, const uint8_t *in_u
     if (n_bytes == 0) return CHIME_BF_OK;
     const int threads = 256;
     const int blocks = (int)std::min<size_t>((n_bytes + threads - 1) / threads, 148 * 16);
-    chime::unpack_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(in_u8, n_bytes, out_re_im);
+    chime4::unpack_debug_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(in_u8, n_bytes, out_re_im);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
         set_err("debug_unpack: %s", cudaGetErrorString(e));
@@ -859,7 +742,7 @@ size_t chime_bf_in_bytes(const chime_bf_plan *plan) {
 size_t chime_bf_out_elems(const chime_bf_plan *plan) {
     return plan ? (size_t)plan->C * plan->R * 1024 * 16 : 0;
 }
-int chime_bf_launches_per_execute(const chime_bf_plan *plan) { return plan ? plan->n_pass : 0; }   // execute_host: one per channel
+int chime_bf_launches_per_execute(const chime_bf_plan *plan) { return plan ? 1 : 0; }   // execute_host: one per chunk
 
 void chime_bf_destroy(chime_bf_plan *pl) {
     if (!pl) return;
@@ -868,7 +751,6 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_slot_of_m);
     cudaFree(pl->d_tw_np);
     cudaFree(pl->d_tw_u);
-    cudaFree(pl->d_bfrag);
     cudaFree(pl->d_stage_in);
     cudaFree(pl->d_stage_out);
     cudaFree(pl->d_delay);

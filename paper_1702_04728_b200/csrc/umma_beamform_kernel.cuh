@@ -41,7 +41,7 @@
 #include <stdint.h>
 
 #include "beamform_kernel.cuh"       // chime::beam_major_dst
-#include "beamform_mma_kernel.cuh"   // chime2::int_bfly4, time_pretwiddle, c_tw128
+#include "int_butterflies.cuh"       // chime4::int_bfly4, c_tw128
 #include "fft_regs.cuh"
 
 namespace chime4 {
@@ -50,7 +50,7 @@ using chime::bitrev;
 using chime::fft_dif;
 
 constexpr int kThreads = 768;
-constexpr int kChunkFrames = 4;                 // output frames per item (their intensities live in registers)
+constexpr int kMaxChunkFrames = 16;             // most output frames per item (polarisation-0 sums wait in the scratch)
 constexpr int kRawBytes = 128 * 256;            // one (block, pol, cylinder): 32 KiB
 constexpr int kBopBytes = 64 * 512;             // one B tile: 64 columns x K 512 bytes
 constexpr int kRecvBytes = 4 * 2 * 8 * 32 * 16; // one receive slot: [cyl][res][i pair][beam][2 x float2] = 32 KiB
@@ -79,6 +79,7 @@ struct Params {
     int n_time, n_frames;
     int chan0, n_chan;        // channel range of this launch
     int frame0, n_frames_launch;
+    int chunk_frames;         // output frames per work item (<= kMaxChunkFrames): weights are reloaded twice per item
     uint8_t *const *peer_out; // beam-major exchange (chime::beam_major_dst), nullptr = off
     int n_peers, chan_global0;
     float norm, scale, offset;
@@ -178,13 +179,6 @@ __device__ __forceinline__ bool elect_one() {
 }
 __device__ __forceinline__ void bar_sync_named(int id, int n) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(n) : "memory"); }
 
-// ---- a1: the nibble split of the packed baseband, four inputs per register ---------------------------------------
-// byte = ((re + 8) << 4) | (im + 8)  ->  offset-binary real parts and imaginary parts, one per byte
-__device__ __forceinline__ void split_nibbles(uint32_t w, uint32_t &re_off, uint32_t &im_off) {
-    re_off = (w >> 4) & 0x0F0F0F0Fu;
-    im_off = w & 0x0F0F0F0Fu;
-}
-
 // ---- operand preparation: one tile (residue pair) of one raw block ----------------------------------------------
 // TT = 0: columns A_0, A_4; 1: A_2, A_6; 2: E_1, O'_1; 3: E_3, O'_3.  B tile row n = 32 variant + 16 set + u',
 // K byte 32 j + i (i < 16): first half of feed 16 j + i, 32 j + 16 + i: second half; variant 0 = [re | im],
@@ -210,8 +204,8 @@ __device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned cha
 #pragma unroll
             for (int k = 0; k < 8; ++k) t[k] = w == 0 ? q[k].x : w == 1 ? q[k].y : w == 2 ? q[k].z : q[k].w;
             uint32_t er, ei, orr, oi;
-            chime2::int_bfly4<R4>(t[0], t[2], t[4], t[6], er, ei);     // bytes = value + 32
-            chime2::int_bfly4<R4>(t[1], t[3], t[5], t[7], orr, oi);
+            int_bfly4<R4>(t[0], t[2], t[4], t[6], er, ei);     // bytes = value + 32
+            int_bfly4<R4>(t[1], t[3], t[5], t[7], orr, oi);
             if constexpr (TT == 0) {          // A_0 = E + O, A_4 = E - O
                 re0[w] = er + orr;          im0[w] = ei + oi;
                 re1[w] = (er + H40) - orr;  im1[w] = (ei + H40) - oi;
@@ -389,7 +383,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
     asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory");
     const uint32_t tb = *s_tmem;
 
-    const int n_chunks = (prm.n_frames_launch + kChunkFrames - 1) / kChunkFrames;
+    const int n_chunks = (prm.n_frames_launch + prm.chunk_frames - 1) / prm.chunk_frames;
     const int n_items = prm.n_chan * n_chunks * 2;
     int *const status = prm.status;
     long long prof_w[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -400,8 +394,8 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
     for (int item = cluster_id; item < n_items; item += n_clusters) {                      \
         const int rt = item & 1, chunk = (item >> 1) % n_chunks;                           \
         const int c = prm.chan0 + (item >> 1) / n_chunks;                                  \
-        const int fr0 = prm.frame0 + chunk * kChunkFrames;                                 \
-        const int nf = min(kChunkFrames, prm.frame0 + prm.n_frames_launch - fr0);          \
+        const int fr0 = prm.frame0 + chunk * prm.chunk_frames;                                \
+        const int nf = min(prm.chunk_frames, prm.frame0 + prm.n_frames_launch - fr0);         \
         (void)rt; (void)c; (void)fr0; (void)nf;
 
     // Register budget per warpgroup: 32 / 80 / 112 / 112 / 72 / 72.  setmaxnreg only redistributes what the CTA was
@@ -582,7 +576,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
 #pragma unroll
         for (int s = 0; s < 4; ++s) sf_remote[s] = mapa(BAR(B_SLOT_FREE + 2 * rank), s);
         float *ost = reinterpret_cast<float *>(smem + kOfsOut) + (e2 * 32 + lane) * 17;
-        float4 *scr = reinterpret_cast<float4 *>(prm.scratch + ((size_t)blockIdx.x * kChunkFrames * 128 + e2 * 32 + lane) * 16);
+        float4 *scr = reinterpret_cast<float4 *>(prm.scratch + ((size_t)blockIdx.x * kMaxChunkFrames * 128 + e2 * 32 + lane) * 16);
         uint32_t tau = 0;
         ITEM_LOOP
             float2 be[4];
@@ -640,7 +634,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                             const int tt = t & 3;
                             const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
 #pragma unroll
-                            for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], chime2::c_tw128[(rho * u) & 127]);
+                            for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_tw128[(rho * u) & 127]);
                             fft_dif<16>(a);
 #pragma unroll
                             for (int i = 0; i < 16; ++i) {
