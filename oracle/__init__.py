@@ -221,3 +221,49 @@ def dedisperse(I, delays):
             d = int(delays[c, g])
             D += I[c, d:d + n_out, :, g].astype(acc_t).T
     return D
+
+
+# ---- exact chromatic alignment (section 4: beam interpolation) -----------------------------------
+def ns_turns(f_mhz, fref_mhz=F_REF_MHZ, sin_theta=None, n_feed=N_FEED, feed_spacing_m=FEED_SPACING_M):
+    """Phase step per feed, in cycles, of the 256 desired pointings at frequency f: f d sin(theta_m) / c0.
+    Native grid (reading A2): sin(theta_m) = (m - N/2) c0 / (N d f_ref), i.e. turns = (m - N/2) f / (N f_ref)."""
+    if sin_theta is None:
+        m = np.arange(n_feed, dtype=np.float64) - n_feed // 2
+        return (m * float(f_mhz)) / (float(n_feed) * float(fref_mhz))
+    s = np.ascontiguousarray(sin_theta, dtype=np.float64)
+    return (float(f_mhz) * 1e6) * (feed_spacing_m / C0) * s
+
+
+def beamform_exact(x, g, turns, w_ew):
+    """Steps 2-4 with the N-S phase of the desired pointing itself (no nearest bin).  Shapes as `beamform`."""
+    n_t, n_pol, n_cyl, n_feed = x.shape
+    turns = np.ascontiguousarray(turns, dtype=np.float64)
+    n_ew = w_ew.shape[0]
+    xd, gd = _c2d(x), _c2d(g)
+    w = np.ascontiguousarray(w_ew, dtype=np.float64)
+    Z = np.zeros((n_t, n_pol, n_ew, turns.size, 2), dtype=np.float64)
+    i = ctypes.c_int
+    lib().oracle_beamform_exact(_p(xd, ctypes.c_double), _p(gd, ctypes.c_double), i(n_t), i(n_pol), i(n_cyl),
+                                i(n_feed), _p(turns, ctypes.c_double), i(turns.size), i(n_ew),
+                                _p(w, ctypes.c_double), _p(Z, ctypes.c_double))
+    return Z.view(np.complex128)[..., 0]
+
+
+def cell_exact(in_u8_cell, f_mhz, gains=None, U=128, ew_deg=EW_ANGLES_DEG, fref_mhz=F_REF_MHZ, sin_theta=None,
+               cyl_spacing_m=CYL_SPACING_M):
+    """One (channel, output frame) cell with exact pointing, steps 1-6.  Returns I [4][256][16] float64."""
+    b = np.ascontiguousarray(in_u8_cell, dtype=np.uint8)
+    assert b.shape == (N_INT * U, N_POL * N_CYL * N_FEED), b.shape
+    turns = np.ascontiguousarray(ns_turns(f_mhz, fref_mhz, sin_theta), dtype=np.float64)
+    w = np.ascontiguousarray(ew_weights(f_mhz, ew_deg, N_CYL, cyl_spacing_m), dtype=np.float64)
+    gp = None
+    if gains is not None:
+        gains = np.ascontiguousarray(gains, dtype=np.float32)
+        assert gains.shape == (N_POL * N_CYL * N_FEED, 2)
+        gp = _p(gains, ctypes.c_float)
+    I = np.zeros((N_EW, turns.size, N_FINE), dtype=np.float64)
+    i = ctypes.c_int
+    lib().oracle_cell_from_u8_exact(_p(b, ctypes.c_uint8), gp, i(N_POL), i(N_CYL), i(N_FEED),
+                                    _p(turns, ctypes.c_double), i(turns.size), i(N_EW), _p(w, ctypes.c_double),
+                                    i(U), i(N_INT), i(N_FINE), _p(I, ctypes.c_double))
+    return I

@@ -284,3 +284,82 @@ void oracle_cell_from_u8(const uint8_t *in_u8, const float *gains, int n_pol, in
     free(x);
     free(g);
 }
+
+/*
+ * Exact chromatic alignment (section 4: "beam interpolation, which would enable the
+ * FFT-formed beams to be perfectly aligned across observing frequencies"; added after the steps
+ * above, which it leaves untouched).  Step 3 with the nearest-bin phase J[m] n / NP replaced by
+ * the phase of the desired pointing itself:
+ *     Y[m] = sum_n v[n] exp(-2 pi i n turns[m]),   turns[m] = f d sin(theta_m) / c0
+ * (cycles of phase per feed; for the native grid of reading A2, turns[m] = (m - N/2) f / (N f_ref)).
+ * Everything else (steps 2, 4) as in oracle_beamform.  The argument n * turns is reduced to
+ * [-1/2, 1/2) before cos/sin.
+ */
+void oracle_beamform_exact(const double *x, const double *g, int n_t, int n_pol, int n_cyl,
+                           int n_feed, const double *turns, int n_beam, int n_ew,
+                           const double *w_ew, double *Z) {
+    cplx *tw = (cplx *)malloc(sizeof(cplx) * (size_t)n_beam * n_feed);
+    for (int m = 0; m < n_beam; ++m)
+        for (int n = 0; n < n_feed; ++n) {
+            double ph = (double)n * turns[m];
+            ph -= floor(ph + 0.5);
+            tw[(size_t)m * n_feed + n].re = cos(-2.0 * ORACLE_PI * ph);
+            tw[(size_t)m * n_feed + n].im = sin(-2.0 * ORACLE_PI * ph);
+        }
+    const cplx *X = (const cplx *)x;
+    const cplx *G = (const cplx *)g;
+    const cplx *W = (const cplx *)w_ew;
+    cplx *Zc = (cplx *)Z;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int t = 0; t < n_t; ++t)
+        for (int p = 0; p < n_pol; ++p) {
+            const cplx *xr = X + ((size_t)t * n_pol + p) * n_cyl * n_feed;
+            const cplx *gr = G + (size_t)p * n_cyl * n_feed;
+            for (int e = 0; e < n_ew; ++e)
+                for (int m = 0; m < n_beam; ++m) {
+                    cplx z = { 0.0, 0.0 };
+                    for (int c = 0; c < n_cyl; ++c) {
+                        cplx y = { 0.0, 0.0 };
+                        for (int n = 0; n < n_feed; ++n) {
+                            cplx pr = cmul(cmul(gr[c * n_feed + n], xr[c * n_feed + n]),
+                                           tw[(size_t)m * n_feed + n]);
+                            y.re += pr.re;
+                            y.im += pr.im;
+                        }
+                        cplx pr = cmul(W[e * n_cyl + c], y);
+                        z.re += pr.re;
+                        z.im += pr.im;
+                    }
+                    Zc[(((size_t)t * n_pol + p) * n_ew + e) * n_beam + m] = z;
+                }
+        }
+    free(tw);
+}
+
+/* One output cell from packed baseband with exact pointing: steps 1, 2, 3 (exact), 4, 5, 6. */
+void oracle_cell_from_u8_exact(const uint8_t *in_u8, const float *gains, int n_pol, int n_cyl,
+                               int n_feed, const double *turns, int n_beam, int n_ew,
+                               const double *w_ew, int U, int n_int, int n_fine, double *I_out) {
+    int n_t = n_int * U;
+    size_t n_in = (size_t)n_pol * n_cyl * n_feed;
+    double *x = (double *)malloc(sizeof(double) * 2 * n_t * n_in);
+    double *g = (double *)malloc(sizeof(double) * 2 * n_in);
+    for (size_t i = 0; i < (size_t)n_t * n_in; ++i) {
+        int8_t ri[2];
+        oracle_unpack(in_u8 + i, 1, ri);
+        x[2 * i] = (double)ri[0];
+        x[2 * i + 1] = (double)ri[1];
+    }
+    for (size_t i = 0; i < n_in; ++i) {
+        g[2 * i] = gains ? (double)gains[2 * i] : 1.0;
+        g[2 * i + 1] = gains ? (double)gains[2 * i + 1] : 0.0;
+    }
+    size_t nz = (size_t)n_t * n_pol * n_ew * n_beam;
+    double *Z = (double *)malloc(sizeof(double) * 2 * nz);
+    oracle_beamform_exact(x, g, n_t, n_pol, n_cyl, n_feed, turns, n_beam, n_ew, w_ew, Z);
+    double norm = 1.0 / ((double)n_feed * (double)n_cyl * (double)U);
+    oracle_upchan_detect(Z, n_int, U, n_pol, n_ew * n_beam, n_fine, norm, I_out, NULL);
+    free(Z);
+    free(x);
+    free(g);
+}

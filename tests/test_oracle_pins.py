@@ -375,3 +375,80 @@ def test_p14_frequency_summed_beam_width_sec31(orc):
     assert abs(v_zen - gold["fwhm_zenith_deg"]) < 0.2 * gold["fwhm_zenith_deg"]
     assert abs(v_low - gold["fwhm_10deg_elevation_deg"]) < 0.2 * gold["fwhm_10deg_elevation_deg"]
     assert 0.28 < p_zen < 0.36          # 0.886 lambda / D at the band's power-weighted mean wavelength
+
+
+# ---- exact chromatic alignment: oracle.beamform_exact / cell_exact ---------------------------------
+def test_exact_pointing_brute_force_tiny():
+    """P15a: literal cexp triple loop on a tiny array (3 samples, 1 pol, 2 cylinders, 5 feeds, 4 pointings)."""
+    import cmath
+    import oracle
+    rng = np.random.default_rng(31)
+    x = rng.normal(size=(3, 1, 2, 5)) + 1j * rng.normal(size=(3, 1, 2, 5))
+    g = rng.normal(size=(1, 2, 5)) + 1j * rng.normal(size=(1, 2, 5))
+    turns = np.array([-0.31, 0.0, 0.123456, 0.49])
+    w = rng.normal(size=(2, 2)) + 1j * rng.normal(size=(2, 2))
+    Z = oracle.beamform_exact(x, g, turns, np.stack([w.real, w.imag], axis=-1))
+    for t in range(3):
+        for e in range(2):
+            for m in range(4):
+                acc = 0
+                for c in range(2):
+                    y = sum(g[0, c, n] * x[t, 0, c, n] * cmath.exp(-2j * cmath.pi * n * turns[m]) for n in range(5))
+                    acc += w[e, c] * y
+                assert abs(Z[t, 0, e, m] - acc) < 1e-12
+
+
+def test_exact_pointing_equals_nearest_bin_where_the_bin_is_exact():
+    """P15b: at f = f_ref the desired pointings ARE bins of the padded transform (J = P (m - 128)), so the exact
+    and the nearest-bin beamformers are the same sums."""
+    import oracle
+    rng = np.random.default_rng(32)
+    x = rng.normal(size=(2, 2, 4, 256)) + 1j * rng.normal(size=(2, 2, 4, 256))
+    g = np.ones((2, 4, 256), dtype=complex)
+    w = oracle.ew_weights(600.0)
+    J = oracle.ns_index(600.0, 512)
+    Za = oracle.beamform(x, g, J, w, 512)
+    Zb = oracle.beamform_exact(x, g, oracle.ns_turns(600.0), w)
+    assert np.abs(Za - Zb).max() < 1e-9 * np.abs(Za).max()
+
+
+def test_exact_pointing_full_gain_on_target_and_convergence_with_padding():
+    """P15c: a plane wave from the desired pointing of beam m is received with the full gain N A by the exact
+    beamformer (Dirichlet kernel at zero offset) at ANY frequency; the nearest-bin beamformer loses
+    |sin(pi N d)/(N sin(pi d))| with d = turns - J/NP, and converges to the exact one as the padding factor grows
+    (the padding trades cost against beam sensitivity)."""
+    import oracle
+    f, m = 437.5, 201
+    turns = oracle.ns_turns(f)
+    n = np.arange(256)
+    x = np.zeros((1, 1, 1, 256), dtype=complex)
+    x[0, 0, 0] = 2.5 * np.exp(2j * np.pi * n * turns[m])
+    g = np.ones((1, 1, 256), dtype=complex)
+    w = np.array([[[1.0, 0.0]]])
+    Ze = oracle.beamform_exact(x, g, turns, w)[0, 0, 0]
+    assert abs(abs(Ze[m]) - 256 * 2.5) < 1e-9
+    assert np.argmax(np.abs(Ze)) == m
+    prev = None
+    for P in (1, 2, 4, 8, 32):
+        J = oracle.ns_index(f, 256 * P)
+        Zn = oracle.beamform(x, g, J, w, 256 * P)[0, 0, 0]
+        d = turns[m] - J[m] / (256.0 * P)
+        d -= np.rint(d)
+        closed = 256 * 2.5 if d == 0 else 2.5 * abs(np.sin(np.pi * 256 * d) / np.sin(np.pi * d))
+        assert abs(abs(Zn[m]) - closed) < 1e-8
+        loss = 1.0 - abs(Zn[m]) / (256 * 2.5)
+        assert loss >= -1e-12
+        if prev is not None and P >= 4:
+            assert loss <= prev + 1e-12
+        prev = loss
+    assert prev < 2e-3          # P = 32: the nearest bin is within 1/64 of a native beam spacing
+
+
+def test_cell_exact_matches_cell_at_fref():
+    """P15d: the packed-baseband entry point with exact pointing reduces to oracle.cell at f = f_ref."""
+    import oracle
+    import synth
+    b = synth.noise_bytes(3, 1, 384).numpy()[0]
+    Ia, _ = oracle.cell(b, 600.0)
+    Ib = oracle.cell_exact(b, 600.0)
+    assert np.abs(Ia - Ib).max() < 1e-9 * Ia.max()
