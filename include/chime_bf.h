@@ -76,6 +76,12 @@ typedef struct {
     float scale, offset;         /* u8 = sat(rne(I*scale + offset)); scale <= 0 -> 1/64, 128 */
     double feed_spacing_m;       /* <= 0 -> 0.3048 */
     double cyl_spacing_m;        /* <= 0 -> 22 */
+    int exact_pointing;          /* 0: nearest bin of the zero-padded transform.
+                                    1: exact chromatic alignment ("beam interpolation"): beam m is phased
+                                    to its desired pointing itself, exp(-2 pi i n f d sin(theta_m) / c0); zero_pad then
+                                    only defines the index table that chime_bf_get_ns_index reports.  upchan_len 128
+                                    only (the tensor-core N-S transform takes any steering vector);
+                                    CHIME_BF_E_UNSUPPORTED (NULL plan) otherwise. */
 } chime_bf_params;
 
 chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *params);
@@ -182,6 +188,21 @@ int chime_bf_n_frames(const chime_bf_plan *plan);       /* n_time / (3U) */
 size_t chime_bf_in_bytes(const chime_bf_plan *plan);    /* C * n_time * 2048 */
 size_t chime_bf_out_elems(const chime_bf_plan *plan);   /* C * n_frames * 1024 * 16 */
 int chime_bf_launches_per_execute(const chime_bf_plan *plan); /* kernels launched by one execute */
+
+/*
+ * 0 while every kernel of the plan has run its pipeline to the end; non-zero once a hand-over inside the tensor-core
+ * kernel timed out (a protocol bug: the kernel then stops itself with a trap instead of hanging the device, and the
+ * CUDA context reports the launch failure).  Reads a host-mapped word, no CUDA call.
+ */
+int chime_bf_kernel_status(const chime_bf_plan *plan);
+
+/*
+ * The roofline denominator, measured: FP32 throughput of this device ("the FFT flops at FP32 peak").
+ * Runs two register-resident loops (scalar FFMA, packed FFMA2) on every SM for ~n_iter iterations of 256 operations
+ * per thread, timed with CUDA events on `cuda_stream` (synchronises that stream).
+ *   tflops_out  HOST [2]: scalar FFMA, packed FFMA2, in TFLOP/s (2 flop per lane and FMA)
+ */
+int chime_bf_measure_fp32_peak(void *cuda_stream, int n_iter, double *tflops_out);
 
 void chime_bf_destroy(chime_bf_plan *plan); /* NULL-safe */
 

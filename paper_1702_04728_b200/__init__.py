@@ -20,7 +20,7 @@ EXPORTS = [
     "chime_bf_in_bytes", "chime_bf_out_elems", "chime_bf_launches_per_execute", "chime_bf_destroy",
     "chime_bf_last_error", "chime_bf_update_gains", "chime_bf_update_ew_angles", "chime_bf_update_pointings",
     "chime_bf_dedisp_delays", "chime_bf_dedisperse", "chime_bf_execute_beam_major", "chime_bf_dedisperse_beams",
-    "chime_bf_dedisp_delays_ex",
+    "chime_bf_dedisp_delays_ex", "chime_bf_kernel_status", "chime_bf_measure_fp32_peak",
 ]
 
 
@@ -39,6 +39,7 @@ class chime_bf_params(ctypes.Structure):
         ("offset", ctypes.c_float),
         ("feed_spacing_m", ctypes.c_double),
         ("cyl_spacing_m", ctypes.c_double),
+        ("exact_pointing", ctypes.c_int),
     ]
 
 
@@ -85,6 +86,10 @@ def load_library():
     lib.chime_bf_dedisp_delays_ex.argtypes = [vp, ci, ci, ctypes.c_double, ctypes.c_double, vp, ctypes.POINTER(ci)]
     lib.chime_bf_dedisperse_beams.restype = ci
     lib.chime_bf_dedisperse_beams.argtypes = [vp, vp, ci, vp, ci, ci, ci, ctypes.c_double, ctypes.c_double, vp, vp, ci]
+    lib.chime_bf_kernel_status.restype = ci
+    lib.chime_bf_kernel_status.argtypes = [vp]
+    lib.chime_bf_measure_fp32_peak.restype = ci
+    lib.chime_bf_measure_fp32_peak.argtypes = [vp, ci, vp]
     lib.chime_bf_n_frames.restype = ci
     lib.chime_bf_n_frames.argtypes = [vp]
     lib.chime_bf_in_bytes.restype = ctypes.c_size_t
@@ -242,6 +247,10 @@ class Plan:
                                                          in_u8.numel(), out.data_ptr()))
         return out
 
+    def kernel_status(self):
+        """chime_bf_kernel_status: 0 unless a hand-over inside the tensor-core kernel timed out."""
+        return load_library().chime_bf_kernel_status(self._h)
+
     def destroy(self):
         if self._h:
             load_library().chime_bf_destroy(self._h)
@@ -282,6 +291,15 @@ def dedisperse_beams(beams_u8, freq_mhz, dm, upchan_len=128, f_ref_mhz=0.0, stre
     return out
 
 
+def measure_fp32_peak(n_iter=2000, stream=None):
+    """chime_bf_measure_fp32_peak -> (scalar FFMA, packed FFMA2) TFLOP/s of the current device."""
+    out = (ctypes.c_double * 2)()
+    rc = load_library().chime_bf_measure_fp32_peak(_stream_ptr(stream), int(n_iter), out)
+    if rc != 0:
+        raise ChimeBfError(f"chime_bf error {rc}: {last_error()}")
+    return float(out[0]), float(out[1])
+
+
 def plan_create(n_coarse, gains=None, ew_angles=EW_ANGLES_DEG, zero_pad=512, upchan_len=128):
     """chime_bf_plan_create: north-star form (f_k = 800 - k*0.390625 MHz, n_time = 49152)."""
     lib = load_library()
@@ -300,7 +318,7 @@ def plan_create(n_coarse, gains=None, ew_angles=EW_ANGLES_DEG, zero_pad=512, upc
 
 def plan_create_ex(n_coarse, freq_mhz=None, gains=None, ew_angles=EW_ANGLES_DEG, zero_pad=512,
                    upchan_len=128, n_time=49152, f_ref_mhz=0.0, ns_sin_theta=None, scale=0.0, offset=0.0,
-                   feed_spacing_m=0.0, cyl_spacing_m=0.0):
+                   feed_spacing_m=0.0, cyl_spacing_m=0.0, exact_pointing=False):
     """chime_bf_plan_create_ex: every knob of chime_bf_params (zeros select the defaults)."""
     lib = load_library()
     keep = []
@@ -324,6 +342,7 @@ def plan_create_ex(n_coarse, freq_mhz=None, gains=None, ew_angles=EW_ANGLES_DEG,
     p.ns_sin_theta = dptr(ns_sin_theta, N_FEED, ctypes.c_double, np.float64)
     p.scale, p.offset = scale, offset
     p.feed_spacing_m, p.cyl_spacing_m = feed_spacing_m, cyl_spacing_m
+    p.exact_pointing = 1 if exact_pointing else 0
     h = lib.chime_bf_plan_create_ex(ctypes.byref(p))
     if not h:
         raise ChimeBfError(last_error())

@@ -14,6 +14,7 @@
 
 #include "beamform_kernel.cuh"
 #include "dedisperse_kernel.cuh"
+#include "fp32_peak.cuh"
 #include "umma_beamform_kernel.cuh"
 
 namespace {
@@ -43,6 +44,8 @@ struct chime_bf_plan {
     std::vector<double> ns_sin;    // [256] explicit pointings, empty = native grid at fref
     double ew_deg[4] = {0, 0, 0, 0};
     double fref = 600.0, d_feed = 0.3048, d_cyl = 22.0;
+    bool exact_pointing = false;  // steer to the desired pointing itself instead of the nearest bin
+    double *d_turns = nullptr;    // [C][256] phase step per feed (cycles) of the desired pointings, exact pointing only
     float2 *d_wp = nullptr;
     int16_t *d_slot = nullptr;
     int16_t *d_slot_of_m = nullptr;
@@ -220,6 +223,17 @@ bool build_umma_weights(chime_bf_plan *pl, cudaStream_t st) {
     wp.gains = pl->gains.empty() ? nullptr : pl->d_gains;
     wp.J = pl->d_J;
     wp.turns = nullptr;
+    if (pl->exact_pointing) {
+        // turns[m] = f d sin(theta_m) / c0; native grid (reading A2): (m - 128) f / (256 f_ref)
+        std::vector<double> turns((size_t)C * 256);
+        for (int c = 0; c < C; ++c)
+            for (int m = 0; m < 256; ++m)
+                turns[(size_t)c * 256 + m] = !pl->ns_sin.empty()
+                    ? (pl->freq[c] * 1e6) * (pl->d_feed / kC0) * pl->ns_sin[m]
+                    : ((double)(m - 128) * pl->freq[c]) / (256.0 * pl->fref);
+        if (!upload_on(&pl->d_turns, turns, st)) return false;
+        wp.turns = pl->d_turns;
+    }
     wp.scale = pl->d_wscale;
     wp.NP = pl->NP;
     chime4::build_weights_kernel<<<C * 16, 128, 0, st>>>(wp);
@@ -464,6 +478,12 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     pl->scale = p.scale > 0.f ? p.scale : 1.0f / 64.0f;
     pl->offset = p.scale > 0.f ? p.offset : 128.0f;
     pl->norm = (float)(1.0 / (256.0 * 4.0 * (double)p.upchan_len));
+    pl->exact_pointing = p.exact_pointing != 0;
+    if (pl->exact_pointing && p.upchan_len != 128) {
+        set_err("plan_create: exact_pointing needs upchan_len 128");
+        delete pl;
+        return nullptr;
+    }
     pl->use_umma = p.upchan_len == 128;   // upchan 256 runs the fp32 kernel of beamform_kernel.cuh
     cudaGetDevice(&pl->device);
     pl->fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
@@ -727,7 +747,43 @@ int chime_bf_debug_unpack(chime_bf_plan *plan, void *stream, const uint8_t *in_u
     return CHIME_BF_OK;
 }
 
-int chime_bf_debug_status(const chime_bf_plan *plan, int code) { return (plan && plan->h_status && code >= 0 && code < 128) ? plan->h_status[code] : 0; }
+int chime_bf_kernel_status(const chime_bf_plan *plan) {
+    if (!plan || !plan->h_status) return 0;
+    for (int i = 0; i < 128; ++i)
+        if (plan->h_status[i]) return (i >> 3) | (plan->h_status[i] & ~0xFF);   // which wait, warp and tile counter
+    return 0;
+}
+
+int chime_bf_measure_fp32_peak(void *stream, int n_iter, double *tflops_out) {
+    if (!tflops_out || n_iter < 1) { set_err("measure_fp32_peak: bad argument"); return CHIME_BF_E_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, n_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    float *sink = nullptr;
+    cudaEvent_t e0, e1;
+    if (cudaMalloc((void **)&sink, sizeof(float) * 1024) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess ||
+        cudaEventCreate(&e1) != cudaSuccess) { set_err("measure_fp32_peak: allocation failed"); return CHIME_BF_E_CUDA; }
+    const int grid = n_sm * 4, block = 512;
+    for (int packed = 0; packed < 2; ++packed) {
+        float ms = 0.f;
+        for (int rep = 0; rep < 3; ++rep) {   // best of three (the first also warms up)
+            cudaEventRecord(e0, st);
+            if (packed) chime_peak::fp32_peak_kernel<true><<<grid, block, 0, st>>>(n_iter, sink);
+            else chime_peak::fp32_peak_kernel<false><<<grid, block, 0, st>>>(n_iter, sink);
+            cudaEventRecord(e1, st);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { set_err("measure_fp32_peak: %s", cudaGetErrorString(cudaGetLastError())); return CHIME_BF_E_CUDA; }
+            float t = 0.f;
+            cudaEventElapsedTime(&t, e0, e1);
+            if (rep == 0 || t < ms) ms = t;
+        }
+        tflops_out[packed] = (double)grid * block * (double)n_iter * 256.0 * 2.0 / (ms * 1e-3) / 1e12;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    return CHIME_BF_OK;
+}
 
 #ifdef CHIME_PROF
 int chime_bf_debug_prof(long long *host_out) {   // development builds only: per-warp wait cycles of the last launch
@@ -755,6 +811,7 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_stage_out);
     cudaFree(pl->d_delay);
     cudaFree(pl->d_peer_out);
+    cudaFree(pl->d_turns);
     cudaFree(pl->d_scratch);
     cudaFree(pl->d_wq);
     cudaFree(pl->d_rowsum);
