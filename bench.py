@@ -1,11 +1,13 @@
 """bench.py -- one JSON line per run (contract in DESIGN.md "Measurement").
 
 A "step" is one pass of the whole hot path (a1-a10, one chime_bf_execute) over one batch of
-synthetic CHIME-shaped baseband: BASELINE.json configs[1] (4 coarse channels x 49152 samples x 2048
-inputs = 403 MB in, 8.4 MB out) per GPU.  metric = input baseband GB/s (and, beside it, the number of
-coarse channels that rate sustains in real time, 1 channel = 0.8 GB/s).
+synthetic CHIME-shaped baseband.  Default: one channel group of BASELINE.json configs[3] per GPU (128 coarse
+channels x 49152 samples x 2048 inputs = 12.9 GB in, 268 MB out, device-resident); --workload cfg1 = configs[1]
+(4 channels, 403 MB).  metric = input baseband GB/s (and, beside it, the number of coarse channels that rate
+sustains in real time, 1 channel = 0.8 GB/s).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W]          CUDA arm
+  python bench.py [--gpus N] [--steps K] [--warmup W]          CUDA arm (configs[3] channel group)
+  python bench.py --workload cfg1                              CUDA arm on configs[1]
   python bench.py --impl reference ...                         oracle arm (CPU, bounded sample)
   python bench.py --workload cfg3 [--chunks 80]                full-band streaming (configs[3]), 1 GPU
   python bench.py --workload dedisp                            dedispersion kernel (HBM-bound), 1 GPU
@@ -165,20 +167,28 @@ def run_cuda(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     bf.load_library()
 
-    # ---- workload: configs[1], channels sharded over ranks (weak scaling: 4 channels per GPU) ----
+    # ---- workload: channels sharded over ranks (weak scaling: every GPU its own C channels) ----
     cfg = synth.CONFIGS[1]
-    C, T = cfg["n_coarse"], cfg["n_time"]
-    seed = synth.config_seed(1)
+    T = cfg["n_time"]
+    C = synth.CONFIGS[3]["group"] if args.workload == "group" else cfg["n_coarse"]
+    seed = synth.config_seed(3 if args.workload == "group" else 1)
     from paper_1702_04728_b200.sharding import weak_scaling_shard
     chan0, _ = weak_scaling_shard(C, rank)
+    chan0 %= 1024 - C + 1
     freqs = synth.chime_freqs_mhz(C, 1, k0=chan0)
     gains = synth.gains(seed + 1000 * rank, C, flagged_frac=cfg["flagged"])
     plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, zero_pad=args.zero_pad, upchan_len=args.upchan, n_time=T)
     d_in = synth.noise_bytes(seed, C, T, device="cuda", chan0=chan0)
     d_out = torch.empty(plan.out_shape, dtype=torch.uint8, device="cuda")
-    h_in = d_in.cpu().pin_memory()
-    h_out = torch.empty(plan.out_shape, dtype=torch.uint8).pin_memory()
     in_bytes, out_bytes = plan.in_bytes, plan.out_elems
+    # end to end (host buffers through the C-ABI) on the first 4 channels: PCIe moves 403 MB per step in ~8 ms;
+    # the whole 12.9 GB group would only repeat the same PCIe-bound rate 32 times
+    Ce = min(C, cfg["n_coarse"])
+    plan_e = plan if Ce == C else bf.plan_create_ex(Ce, freq_mhz=freqs[:Ce], gains=gains[:Ce], zero_pad=args.zero_pad,
+                                                    upchan_len=args.upchan, n_time=T)
+    h_in = d_in[:Ce].cpu().pin_memory()
+    h_out = torch.empty(plan_e.out_shape, dtype=torch.uint8).pin_memory()
+    e2e_in_bytes, e2e_out_bytes = plan_e.in_bytes, plan_e.out_elems
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -218,18 +228,22 @@ def run_cuda(args):
 
     # ---- end to end through the C-ABI with HOST buffers (H2D + kernel + D2H inside the call) ----
     n_e2e = max(2, min(args.steps, 5))
-    plan.execute_host(h_in, h_out, stream=stream)
+    plan_e.execute_host(h_in, h_out, stream=stream)
     barrier()
     t0 = time.perf_counter()
     g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     g0.record(stream)
     for _ in range(n_e2e):
-        plan.execute_host(h_in, h_out, stream=stream)
+        plan_e.execute_host(h_in, h_out, stream=stream)
     g1.record(stream)
     barrier()
     e2e_ms = g0.elapsed_time(g1)
     clocks = sampler.stop() if rank == 0 else None
-    assert torch.equal(h_out, d_out.cpu()), "host path and device path disagree"
+    assert torch.equal(h_out, d_out[:Ce].cpu()), "host path and device path disagree"
+    status = plan.kernel_status() | plan_e.kernel_status()
+    assert status == 0, f"a pipeline hand-over timed out inside the kernel (status {status})"
+    # the roofline denominator, measured on this device under this run's clocks
+    peak_ffma, peak_ffma2 = bf.measure_fp32_peak(3000, stream=stream) if rank == 0 else (0.0, 0.0)
 
     if dist is not None:
         t = torch.tensor([total_ms, kern_ms, e2e_ms], device="cuda", dtype=torch.float64)
@@ -241,7 +255,7 @@ def run_cuda(args):
         return 0
 
     gbs = world * args.steps * in_bytes / (total_ms * 1e-3) / 1e9
-    e2e_gbs = world * n_e2e * in_bytes / (e2e_ms * 1e-3) / 1e9
+    e2e_gbs = world * n_e2e * e2e_in_bytes / (e2e_ms * 1e-3) / 1e9
     peaks, peak_kind = measured_peaks()
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     fp32_peak = N_SM * LANES * 2 * sm_mhz * 1e6 / 1e12
@@ -257,8 +271,10 @@ def run_cuda(args):
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             tj = json.load(f)
-        if args.zero_pad == 512 and args.upchan == 128:     # the profile is of the default setting
-            traffic, traffic_src = float(tj["dram_bytes_per_launch"]), tj["source"]
+        if args.zero_pad == 512 and args.upchan == 128:     # the profile is of the default setting (cfg1 launch):
+            # scaled to this launch by the algorithmic bytes (traffic is 1.00x algorithmic in the profile)
+            traffic = float(tj["dram_bytes_per_launch"]) * (in_bytes + out_bytes) / float(tj["algorithmic_bytes"])
+            traffic_src = tj["source"]
     except Exception:
         pass
     line = {
@@ -267,25 +283,32 @@ def run_cuda(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "channels_realtime": gbs / GBS_PER_CHANNEL,
         "realtime_fraction_full_band": gbs / (1024 * GBS_PER_CHANNEL),
-        "config": {"workload": "configs[1] single node load per GPU: 4 coarse channels x 49152 samples x "
-                               f"2048 inputs, zero_pad {args.zero_pad}, upchan {args.upchan}, random gains, 2% flagged",
+        "config": {"workload": (f"one channel group of configs[3] (full-band streaming) per GPU: {C} coarse channels x "
+                                if args.workload == "group" else
+                                f"configs[1] single node load per GPU: {C} coarse channels x ") +
+                               f"{T} samples x 2048 inputs, zero_pad {args.zero_pad}, upchan {args.upchan}, "
+                               "random gains, 2% flagged, device-resident",
                    "in_bytes_per_step": in_bytes, "out_bytes_per_step": out_bytes,
-                   "l2": "input (403 MB) larger than L2 (126 MB); no flush needed",
+                   "l2": f"input ({in_bytes / 1e6:.0f} MB) larger than L2 (126 MB); no flush needed",
                    "parallelism": f"channel-sharded x{world}, no collective"},
         "roofline": {"bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s",
                      "frac": ach / fp32_peak, "traffic": traffic,
                      "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
                      "traffic_source": traffic_src, "algorithmic_bytes": in_bytes + out_bytes,
-                     "kernel": (("chime3::beamform_ws_kernel<true>" if args.zero_pad == 256 else
-                                 "chime3::beamform_ws_kernel<false>") if args.upchan == 128
+                     "peak_measured": peak_ffma2, "frac_of_measured": ach / peak_ffma2 if peak_ffma2 else None,
+                     "peak_measured_note": f"chime_bf_measure_fp32_peak in this run: FFMA {peak_ffma:.1f}, FFMA2 "
+                                           f"{peak_ffma2:.1f} TFLOP/s",
+                     "kernel": ("chime4::umma_beamform_kernel" if args.upchan == 128
                                 else "chime::beamform_fused_kernel"), "kernel_ms": kern_ms,
                      "flops_per_chan_sample": fft_flops,
                      "note": f"FP32 peak = 148 SM x 128 lanes x 2 x {sm_mhz:.0f} MHz ({peak_kind} sm_max_mhz); "
                              "nominal FFT flops (5 n log2 n) per BASELINE north_star",
                      "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
                              "peak_kind": peak_kind}},
-        "e2e": {"value": e2e_gbs, "unit": UNIT, "h2d_bytes_per_step": in_bytes,
-                "d2h_bytes_per_step": out_bytes, "steps": n_e2e},
+        "e2e": {"value": e2e_gbs, "unit": UNIT, "h2d_bytes_per_step": e2e_in_bytes,
+                "d2h_bytes_per_step": e2e_out_bytes, "steps": n_e2e,
+                "workload": f"chime_bf_execute_host on the first {Ce} channels of the step (pinned host buffers; "
+                            "PCIe-bound, so more channels would repeat the same rate)"},
         "gpu_launches": args.steps * plan.launches_per_execute,
         "clocks": clocks,
     }
@@ -430,7 +453,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="cfg1", choices=["cfg1", "cfg3", "dedisp"],
+    ap.add_argument("--workload", default="group", choices=["group", "cfg1", "cfg3", "dedisp"],
                     help="cfg1 (default, the contract's step) or cfg3 (full-band streaming, 1 GPU)")
     ap.add_argument("--chunks", type=int, default=80, help="cfg3: full-band chunks to stream")
     ap.add_argument("--zero-pad", type=int, default=512, choices=[256, 512, 1024],
