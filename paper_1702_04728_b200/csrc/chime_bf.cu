@@ -392,10 +392,7 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
     const int n_cta = n_chan * n_fr * 4;
     cudaError_t e = cudaErrorInvalidValue;
     const int P = pl->NP / 256, RAD = pl->U / 32;
-    if (P == 1 && RAD == 4) e = launch<1, 4>(kp, n_cta, st);
-    else if (P == 2 && RAD == 4) e = launch<2, 4>(kp, n_cta, st);
-    else if (P == 4 && RAD == 4) e = launch<4, 4>(kp, n_cta, st);
-    else if (P == 1 && RAD == 8) e = launch<1, 8>(kp, n_cta, st);
+    if (P == 1 && RAD == 8) e = launch<1, 8>(kp, n_cta, st);
     else if (P == 2 && RAD == 8) e = launch<2, 8>(kp, n_cta, st);
     else if (P == 4 && RAD == 8) e = launch<4, 8>(kp, n_cta, st);
     if (e != cudaSuccess) {
@@ -502,8 +499,7 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     if (p.ns_sin_theta) pl->ns_sin.assign(p.ns_sin_theta, p.ns_sin_theta + 256);
     for (int e = 0; e < 4; ++e) pl->ew_deg[e] = p.ew_angles_deg[e];
     bool ok = build_tables(pl);
-    ok = ok && prepare_kernel<1, 4>() && prepare_kernel<2, 4>() && prepare_kernel<4, 4>() &&
-         prepare_kernel<1, 8>() && prepare_kernel<2, 8>() && prepare_kernel<4, 8>();
+    ok = ok && prepare_kernel<1, 8>() && prepare_kernel<2, 8>() && prepare_kernel<4, 8>();
     if (!ok) {
         chime_bf_destroy(pl);
         return nullptr;
