@@ -267,3 +267,22 @@ def cell_exact(in_u8_cell, f_mhz, gains=None, U=128, ew_deg=EW_ANGLES_DEG, fref_
                                     _p(turns, ctypes.c_double), i(turns.size), i(N_EW), _p(w, ctypes.c_double),
                                     i(U), i(N_INT), i(N_FINE), _p(I, ctypes.c_double))
     return I
+
+
+# ---- the packetiser's per-packet rescale (reading F4 of DESIGN.md -- the paper gives no formula) ------
+def packet_quantize(I, beams_per_packet=32):
+    """I [n_ew][n_beam][n_fine] intensities of one (channel, frame).  A packet = `beams_per_packet` consecutive N-S
+    beams x all fine channels of one E-W beam; scale = 16 / sigma (1 if sigma = 0), offset = 128 - mean * scale
+    (population statistics of the packet), u8 = clamp(rne(I * scale + offset), 0, 255).
+    Returns (u8 like I, scale_offset [n_ew][n_beam / beams_per_packet][2])."""
+    I = np.asarray(I, dtype=np.float64)
+    n_ew, n_beam, n_fine = I.shape
+    n_p = n_beam // beams_per_packet
+    P = I.reshape(n_ew, n_p, beams_per_packet * n_fine)
+    mean = P.mean(axis=-1)
+    sd = np.sqrt(((P - mean[..., None]) ** 2).mean(axis=-1))
+    scale = np.where(sd > 0, 16.0 / np.where(sd > 0, sd, 1.0), 1.0)
+    offset = 128.0 - mean * scale
+    x = P * scale[..., None] + offset[..., None]
+    q = np.clip(np.rint(x), 0, 255).astype(np.uint8)        # np.rint rounds half to even, like cvt.rni
+    return q.reshape(I.shape), np.stack([scale, offset], axis=-1)
