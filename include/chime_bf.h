@@ -176,6 +176,18 @@ int chime_bf_dedisperse_beams(void *cuda_stream, const uint8_t *beams_u8, int n_
                               int n_frames, int n_beams, int upchan_len, double dm, double f_ref_mhz,
                               int32_t *delay_scratch, uint32_t *out_u32, int n_out);
 
+/*
+ * chime_bf_execute with the packetiser's per-packet rescale ("rescaled to 8-bit integers ... in a custom
+ * UDP packet format"; the paper gives no formula -- reading F4 of DESIGN.md): a packet is the 32 consecutive N-S beams
+ * x 16 fine channels (512 intensities) of one (channel, frame, E-W beam); its scale and offset follow from its own
+ * data, scale = 16 / sigma (1 if sigma = 0), offset = 128 - mean * scale, u8 = sat(rne(I * scale + offset)), so that
+ * I ~ (u8 - offset) / scale.  Statistics in fp32.  upchan_len 128 only (CHIME_BF_E_UNSUPPORTED otherwise).
+ *   out_u8        DEVICE, as chime_bf_execute
+ *   scale_offset  DEVICE, [C][n_frames][4][8][2] float (scale, offset) per packet, 8-byte aligned, caller-owned
+ */
+int chime_bf_execute_packets(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8, uint8_t *out_u8,
+                             float *scale_offset);
+
 /* Copy of the clamped N-S bin index table J (eq. (1),(2)): HOST out, [C][256] int32. */
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out);
 

@@ -21,6 +21,7 @@ EXPORTS = [
     "chime_bf_last_error", "chime_bf_update_gains", "chime_bf_update_ew_angles", "chime_bf_update_pointings",
     "chime_bf_dedisp_delays", "chime_bf_dedisperse", "chime_bf_execute_beam_major", "chime_bf_dedisperse_beams",
     "chime_bf_dedisp_delays_ex", "chime_bf_kernel_status", "chime_bf_measure_fp32_peak",
+    "chime_bf_execute_packets",
 ]
 
 
@@ -64,6 +65,8 @@ def load_library():
     lib.chime_bf_execute.argtypes = [vp, vp, vp, vp]
     lib.chime_bf_execute_f32.restype = ci
     lib.chime_bf_execute_f32.argtypes = [vp, vp, vp, vp]
+    lib.chime_bf_execute_packets.restype = ci
+    lib.chime_bf_execute_packets.argtypes = [vp, vp, vp, vp, vp]
     lib.chime_bf_execute_host.restype = ci
     lib.chime_bf_execute_host.argtypes = [vp, vp, vp, vp]
     lib.chime_bf_get_ns_index.restype = ci
@@ -166,6 +169,19 @@ class Plan:
         self._check(load_library().chime_bf_execute_f32(self._h, _stream_ptr(stream), in_u8.data_ptr(),
                                                         out_f32.data_ptr()))
         return out_f32
+
+    def execute_packets(self, in_u8, out_u8=None, scale_offset=None, stream=None):
+        """chime_bf_execute_packets -> (uint8 beams, float32 (scale, offset) per packet [C][R][4][8][2])."""
+        import torch
+        self._check_in(in_u8)
+        if out_u8 is None:
+            out_u8 = torch.empty(self.out_shape, dtype=torch.uint8, device=in_u8.device)
+        if scale_offset is None:
+            scale_offset = torch.empty((self.n_coarse, self.n_frames, N_EW, 8, 2), dtype=torch.float32, device=in_u8.device)
+        assert scale_offset.is_cuda and scale_offset.dtype == torch.float32 and scale_offset.numel() == self.n_coarse * self.n_frames * 64
+        self._check(load_library().chime_bf_execute_packets(self._h, _stream_ptr(stream), in_u8.data_ptr(),
+                                                            out_u8.data_ptr(), scale_offset.data_ptr()))
+        return out_u8, scale_offset
 
     def execute_host(self, in_u8_host, out_u8_host=None, stream=None):
         """HOST tensors (ideally pinned) in and out; H2D, kernels and D2H all inside the call."""

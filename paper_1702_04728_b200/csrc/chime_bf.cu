@@ -319,7 +319,7 @@ cudaError_t launch(const chime::KernelParams &kp, int n_cta, cudaStream_t st) {
 
 int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, float *out_f32, int chan0 = 0,
         int n_chan = -1, int frame0 = 0, int n_fr = -1, uint8_t *const *peer_out = nullptr, int n_peers = 0,
-        int chan_global0 = 0) {
+        int chan_global0 = 0, float *packet_so = nullptr) {
     if (pl && n_chan < 0) n_chan = pl->C;
     if (pl && n_fr < 0) n_fr = pl->R;
     if (!pl || !in || (!out_u8 && !out_f32 && !peer_out)) {
@@ -374,6 +374,7 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         up.offset = pl->offset;
         up.status = pl->d_status;
         up.scratch = pl->d_scratch;
+        up.packet_so = reinterpret_cast<float2 *>(packet_so);
         // frames per work item: as many as possible (the weights are reloaded twice per item), while the launch still
         // has at least 8 items per cluster to balance the persistent grid
         int chunk = chime4::kMaxChunkFrames;
@@ -522,6 +523,14 @@ chime_bf_plan *chime_bf_plan_create(int n_coarse, const float *gains, const doub
 
 int chime_bf_execute(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, uint8_t *out_u8) {
     return run(plan, stream, in_u8, out_u8, nullptr);
+}
+
+int chime_bf_execute_packets(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, uint8_t *out_u8,
+                             float *scale_offset) {
+    if (!plan || !scale_offset || !out_u8) { set_err("execute_packets: null argument"); return CHIME_BF_E_INVALID_ARG; }
+    if (!plan->use_umma) { set_err("execute_packets: upchan_len 128 only"); return CHIME_BF_E_UNSUPPORTED; }
+    if ((uintptr_t)scale_offset & 7) { set_err("execute_packets: scale_offset must be 8-byte aligned"); return CHIME_BF_E_ALIGNMENT; }
+    return run(plan, stream, in_u8, out_u8, nullptr, 0, -1, 0, -1, nullptr, 0, 0, scale_offset);
 }
 
 int chime_bf_execute_f32(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, float *out_f32) {

@@ -83,6 +83,7 @@ struct Params {
     uint8_t *const *peer_out; // beam-major exchange (chime::beam_major_dst), nullptr = off
     int n_peers, chan_global0;
     float norm, scale, offset;
+    float2 *packet_so;        // per-packet (scale, offset) out, [C][R][4 e][8 blocks of 32 beams], or nullptr (fixed scale)
     float *scratch;           // [grid][4 frames][4 e][32 beams][16]: polarisation-0 sums parked until pol 1 is done (L2)
     int *status;              // set to non-zero when a wait timed out (the kernel traps afterwards)
 };
@@ -676,13 +677,34 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
 #pragma unroll
                                 for (int k = 0; k < 4; ++k) dst[k] = make_float4(acc[4 * k], acc[4 * k + 1], acc[4 * k + 2], acc[4 * k + 3]);
                             } else {
+                                float qs = prm.scale, qo = prm.offset;
+                                if (prm.packet_so != nullptr) {
+                                    // per-packet rescale (reading F4): packet = this warp's 32 beams x 16 fine
+                                    // channels of (channel, frame, E-W beam); scale = 16 / sigma, offset = 128 - mean scale
+                                    float s1 = 0.f;
+#pragma unroll
+                                    for (int g = 0; g < 16; ++g) s1 += acc[g];
+#pragma unroll
+                                    for (int o = 16; o > 0; o >>= 1) s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+                                    const float mean = s1 * (1.0f / 512.0f);
+                                    float s2 = 0.f;
+#pragma unroll
+                                    for (int g = 0; g < 16; ++g) s2 = fmaf(acc[g] - mean, acc[g] - mean, s2);
+#pragma unroll
+                                    for (int o = 16; o > 0; o >>= 1) s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+                                    const float sd = sqrtf(s2 * (1.0f / 512.0f));
+                                    qs = sd > 0.f ? 16.0f / sd : 1.0f;
+                                    qo = fmaf(-mean, qs, 128.0f);
+                                    if (lane == 0)
+                                        prm.packet_so[(((size_t)c * prm.n_frames + Rf) * 4 + e2) * 8 + (ns >> 5)] = make_float2(qs, qo);
+                                }
                                 uint32_t qw[4];
 #pragma unroll
                                 for (int k = 0; k < 4; ++k) {
                                     uint32_t word = 0;
 #pragma unroll
                                     for (int b = 0; b < 4; ++b) {
-                                        const float x = fmaf(acc[4 * k + b], prm.scale, prm.offset);
+                                        const float x = fmaf(acc[4 * k + b], qs, qo);
                                         word |= (uint32_t)__float2int_rn(fminf(fmaxf(x, 0.f), 255.f)) << (8 * b);
                                     }
                                     qw[k] = word;
