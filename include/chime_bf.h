@@ -188,6 +188,22 @@ int chime_bf_dedisperse_beams(void *cuda_stream, const uint8_t *beams_u8, int n_
 int chime_bf_execute_packets(chime_bf_plan *plan, void *cuda_stream, const uint8_t *in_u8, uint8_t *out_u8,
                              float *scale_offset);
 
+/*
+ * Dedispersion ACROSS execute buffers (PAPER.md:86 asks for "a high nominal DM": at DM 500 the sweep over the band is
+ * 9.7 s, ten execute buffers of configs[2]).  _begin fixes DM and reference (as chime_bf_dedisp_delays), allocates /
+ * clears a plan-owned ring of partial sums [1024][max delay + n_frames] uint32 and restarts the stream at frame 0
+ * (synchronises `cuda_stream`); *max_delay (may be NULL) = largest delay in frames.  Every _push adds one more buffer
+ * of uint8 beams [C][n_frames][1024][16] (frames t0 .. t0 + n_frames - 1 of the stream, t0 = n_frames x the number of
+ * earlier pushes) and hands out the n_frames dedispersed samples that are complete with it:
+ *   out_u32       DEVICE, [1024][n_frames]: out[b][s] = D[b][*first_sample + s], D[b][r] = sum_c sum_g I[c][r + delay[c][g]][b][g]
+ *                 over the whole stream; samples with a negative index (before the stream starts) are 0
+ *   first_sample  HOST (may be NULL): t0 - max delay
+ * Asynchronous on `cuda_stream` (two kernels), exact in uint32.
+ */
+int chime_bf_dedisperse_stream_begin(chime_bf_plan *plan, void *cuda_stream, double dm, double f_ref_mhz, int *max_delay);
+int chime_bf_dedisperse_stream_push(chime_bf_plan *plan, void *cuda_stream, const uint8_t *beams_u8, uint32_t *out_u32,
+                                    long long *first_sample);
+
 /* Copy of the clamped N-S bin index table J (eq. (1),(2)): HOST out, [C][256] int32. */
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out);
 

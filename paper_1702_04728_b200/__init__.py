@@ -21,7 +21,7 @@ EXPORTS = [
     "chime_bf_last_error", "chime_bf_update_gains", "chime_bf_update_ew_angles", "chime_bf_update_pointings",
     "chime_bf_dedisp_delays", "chime_bf_dedisperse", "chime_bf_execute_beam_major", "chime_bf_dedisperse_beams",
     "chime_bf_dedisp_delays_ex", "chime_bf_kernel_status", "chime_bf_measure_fp32_peak",
-    "chime_bf_execute_packets",
+    "chime_bf_execute_packets", "chime_bf_dedisperse_stream_begin", "chime_bf_dedisperse_stream_push",
 ]
 
 
@@ -65,6 +65,10 @@ def load_library():
     lib.chime_bf_execute.argtypes = [vp, vp, vp, vp]
     lib.chime_bf_execute_f32.restype = ci
     lib.chime_bf_execute_f32.argtypes = [vp, vp, vp, vp]
+    lib.chime_bf_dedisperse_stream_begin.restype = ci
+    lib.chime_bf_dedisperse_stream_begin.argtypes = [vp, vp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ci)]
+    lib.chime_bf_dedisperse_stream_push.restype = ci
+    lib.chime_bf_dedisperse_stream_push.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_longlong)]
     lib.chime_bf_execute_packets.restype = ci
     lib.chime_bf_execute_packets.argtypes = [vp, vp, vp, vp, vp]
     lib.chime_bf_execute_host.restype = ci
@@ -249,6 +253,25 @@ class Plan:
         self._check(load_library().chime_bf_dedisperse(self._h, _stream_ptr(stream), beams_u8.data_ptr(),
                                                        float(dm), float(f_ref_mhz), out_u32.data_ptr(), n_out))
         return out_u32
+
+    def dedisperse_stream_begin(self, dm, f_ref_mhz=0.0, stream=None):
+        """chime_bf_dedisperse_stream_begin -> largest delay in frames."""
+        mx = ctypes.c_int(0)
+        self._check(load_library().chime_bf_dedisperse_stream_begin(self._h, _stream_ptr(stream), float(dm),
+                                                                    float(f_ref_mhz), ctypes.byref(mx)))
+        return mx.value
+
+    def dedisperse_stream_push(self, beams_u8, out_u32=None, stream=None):
+        """chime_bf_dedisperse_stream_push -> (int32 [1024][n_frames], stream index of its first sample)."""
+        import torch
+        assert beams_u8.is_cuda and beams_u8.dtype == torch.uint8 and beams_u8.is_contiguous()
+        assert beams_u8.numel() == self.out_elems
+        if out_u32 is None:
+            out_u32 = torch.empty((N_BEAM, self.n_frames), dtype=torch.int32, device=beams_u8.device)
+        first = ctypes.c_longlong(0)
+        self._check(load_library().chime_bf_dedisperse_stream_push(self._h, _stream_ptr(stream), beams_u8.data_ptr(),
+                                                                   out_u32.data_ptr(), ctypes.byref(first)))
+        return out_u32, first.value
 
     def get_ns_index(self):
         J = np.zeros((self.n_coarse, N_FEED), dtype=np.int32)

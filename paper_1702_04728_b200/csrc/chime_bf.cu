@@ -60,6 +60,11 @@ struct chime_bf_plan {
     int host_parts = 1;                   // execute_host: frame ranges per channel
     uint8_t **d_peer_out = nullptr;       // execute_beam_major: device copy of the peers' receive-buffer pointers (<= 64)
     int32_t *d_delay = nullptr;   // [C][16] dedispersion delays of the last chime_bf_dedisperse call
+    // streaming dedispersion (chime_bf_dedisperse_stream_begin / _push): ring of partial sums across execute buffers
+    uint32_t *d_ring = nullptr;   // [1024][dd_L]
+    int32_t *d_delay_stream = nullptr;
+    int dd_D = -1, dd_L = 0;
+    long long dd_t0 = 0;
     // tensor-core N-S path (umma_beamform_kernel.cuh; upchan_len 128, any zero_pad)
     bool use_umma = false;
     uint32_t *d_wq = nullptr;     // TMEM images of the three-digit integer weights, 3 MiB per channel
@@ -687,6 +692,62 @@ int chime_bf_dedisperse(chime_bf_plan *pl, void *stream, const uint8_t *beams_u8
     return launch_dedisperse(stream, beams_u8, pl->C, pl->R, 1024, tab, pl->d_delay, out_u32, n_out);
 }
 
+int chime_bf_dedisperse_stream_begin(chime_bf_plan *pl, void *stream, double dm, double f_ref_mhz, int *max_delay) {
+    if (!pl || !(dm >= 0)) { set_err("dedisperse_stream_begin: bad argument"); return CHIME_BF_E_INVALID_ARG; }
+    std::vector<int32_t> tab;
+    const int D = dedisp_table(pl->freq.data(), pl->C, pl->U, dm, f_ref_mhz, tab);
+    for (int32_t d : tab)
+        if (d < 0) { set_err("dedisperse_stream_begin: f_ref below a fine channel (negative delay)"); return CHIME_BF_E_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const int L = D + pl->R;
+    cudaError_t e = cudaSuccess;
+    if (L > pl->dd_L) {
+        cudaFree(pl->d_ring);
+        pl->d_ring = nullptr;
+        e = cudaMalloc((void **)&pl->d_ring, (size_t)1024 * L * sizeof(uint32_t));
+        pl->dd_L = (e == cudaSuccess) ? L : 0;
+    }
+    if (e == cudaSuccess && !pl->d_delay_stream) e = cudaMalloc((void **)&pl->d_delay_stream, (size_t)pl->C * 16 * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemsetAsync(pl->d_ring, 0, (size_t)1024 * pl->dd_L * sizeof(uint32_t), st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_delay_stream, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // `tab` is a pageable temporary
+    if (e != cudaSuccess) { set_err("dedisperse_stream_begin: %s", cudaGetErrorString(e)); return CHIME_BF_E_CUDA; }
+    pl->dd_D = D;
+    pl->dd_t0 = 0;
+    if (max_delay) *max_delay = D;
+    return CHIME_BF_OK;
+}
+
+int chime_bf_dedisperse_stream_push(chime_bf_plan *pl, void *stream, const uint8_t *beams_u8, uint32_t *out_u32,
+                                    long long *first_sample) {
+    if (!pl || !beams_u8 || !out_u32) { set_err("dedisperse_stream_push: null argument"); return CHIME_BF_E_INVALID_ARG; }
+    if (pl->dd_D < 0) { set_err("dedisperse_stream_push: call chime_bf_dedisperse_stream_begin first"); return CHIME_BF_E_INVALID_ARG; }
+    if ((uintptr_t)beams_u8 & 15) { set_err("dedisperse_stream_push: input must be 16-byte aligned"); return CHIME_BF_E_ALIGNMENT; }
+    chime_dd::StreamParams sp;
+    sp.in = reinterpret_cast<const uint32_t *>(beams_u8);
+    sp.delay = pl->d_delay_stream;
+    sp.ring = pl->d_ring;
+    sp.out = out_u32;
+    sp.C = pl->C;
+    sp.R = pl->R;
+    sp.D = pl->dd_D;
+    sp.L = pl->dd_L;
+    sp.n_beams = 1024;
+    sp.t0 = pl->dd_t0;
+    const int bt = 1024 / chime_dd::kBeamsPerCta, tt = (pl->dd_D + pl->R + chime_dd::kTR - 1) / chime_dd::kTR;
+    int n_split = std::min(pl->C, std::max(1, (148 * 16 + bt * tt - 1) / (bt * tt)));
+    sp.c_per_split = (pl->C + n_split - 1) / n_split;
+    n_split = (pl->C + sp.c_per_split - 1) / sp.c_per_split;
+    cudaStream_t st = (cudaStream_t)stream;
+    chime_dd::dedisperse_stream_kernel<<<dim3(bt, tt, n_split), chime_dd::kThreads, 0, st>>>(sp);
+    chime_dd::dedisperse_emit_kernel<<<dim3((pl->R + 255) / 256, 1024), 256, 0, st>>>(sp);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { set_err("dedisperse_stream_push: %s", cudaGetErrorString(e)); return CHIME_BF_E_CUDA; }
+    if (first_sample) *first_sample = pl->dd_t0 - pl->dd_D;   // stream index of out_u32[.][0]; samples < 0 are zero
+    pl->dd_t0 += pl->R;
+    return CHIME_BF_OK;
+}
+
 int chime_bf_dedisp_delays_ex(const double *freq_mhz, int n_coarse, int upchan_len, double dm, double f_ref_mhz,
                               int32_t *host_out, int *max_delay) {
     if (!freq_mhz || n_coarse < 1 || !(dm >= 0) || (upchan_len != 128 && upchan_len != 256)) {
@@ -815,6 +876,8 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_stage_in);
     cudaFree(pl->d_stage_out);
     cudaFree(pl->d_delay);
+    cudaFree(pl->d_ring);
+    cudaFree(pl->d_delay_stream);
     cudaFree(pl->d_peer_out);
     cudaFree(pl->d_turns);
     cudaFree(pl->d_scratch);

@@ -77,4 +77,75 @@ __global__ void __launch_bounds__(kThreads, 4) dedisperse_kernel(const Params p)
         }
 }
 
+// ---- streaming form: sweeps longer than one execute buffer (PAPER.md:86 asks for a HIGH nominal DM) ------------------
+// A plan-owned ring of partial sums ring[n_beams][L], L >= D + R (D = largest delay).  Buffer number k holds frames
+// t0 .. t0 + R - 1 of the stream (t0 = k R).  With rel = 0 .. D + R - 1 and r = t0 - D + rel the dedispersed sample a
+// ring column stands for, the buffer contributes
+//     ring[b][(t0 + rel) mod L] += sum_{c, g : 0 <= rel - D + delay[c][g] < R} I[c][rel - D + delay[c][g]][b][g];
+// afterwards the columns rel < R are complete (every frame they need has been seen): emit_kernel hands them out and
+// clears them for re-use.  Same thread mapping and one-load-per-distinct-delay scheme as dedisperse_kernel; every
+// input byte is still read once.
+struct StreamParams {
+    const uint32_t *in;      // [C][R][n_beams][4] words
+    const int32_t *delay;    // [C][16]
+    uint32_t *ring;          // [n_beams][L]
+    uint32_t *out;           // [n_beams][R] (emit_kernel)
+    int C, R, D, L, n_beams;
+    long long t0;            // first frame of this buffer in the stream
+    int c_per_split;
+};
+
+__global__ void __launch_bounds__(kThreads, 4) dedisperse_stream_kernel(const StreamParams p) {
+    const int tid = threadIdx.x;
+    const int q = tid & 3;
+    const int b = blockIdx.x * kBeamsPerCta + (tid >> 2);
+    const int rel0 = blockIdx.y * kTR;
+    uint32_t acc[kTR];
+#pragma unroll
+    for (int r = 0; r < kTR; ++r) acc[r] = 0u;
+    const size_t frame_words = (size_t)p.n_beams * 4;
+    const int c_lo = blockIdx.z * p.c_per_split, c_hi = min(p.C, c_lo + p.c_per_split);
+#pragma unroll 1
+    for (int c = c_lo; c < c_hi; ++c) {
+        const int4 dl = *reinterpret_cast<const int4 *>(p.delay + c * 16 + 4 * q);
+        const uint32_t *base = p.in + (size_t)c * p.R * frame_words + (size_t)b * 4 + q;
+        const int v_lo = min(min(dl.x, dl.y), min(dl.z, dl.w)), v_hi = max(max(dl.x, dl.y), max(dl.z, dl.w));
+#pragma unroll 1
+        for (int v = v_lo; v <= v_hi; ++v) {
+            const uint32_t mask = (dl.x == v ? 0x01u : 0u) | (dl.y == v ? 0x0100u : 0u) | (dl.z == v ? 0x010000u : 0u) |
+                                  (dl.w == v ? 0x01000000u : 0u);
+            const int f0 = rel0 - p.D + v;                         // frame (inside this buffer) of the tile's first sample
+            if (mask == 0u || f0 + kTR <= 0 || f0 >= p.R) continue;  // the whole tile lies in another buffer
+            const uint32_t *src = base + (ptrdiff_t)f0 * (ptrdiff_t)frame_words;
+            uint32_t w[kTR];
+#pragma unroll
+            for (int r = 0; r < kTR; ++r) w[r] = ((unsigned)(f0 + r) < (unsigned)p.R) ? __ldg(src + (size_t)r * frame_words) : 0u;
+#pragma unroll
+            for (int r = 0; r < kTR; ++r) acc[r] = __dp4a(w[r], mask, acc[r]);
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < kTR; ++r) {
+        acc[r] += __shfl_xor_sync(0xFFFFFFFFu, acc[r], 1);
+        acc[r] += __shfl_xor_sync(0xFFFFFFFFu, acc[r], 2);
+    }
+    uint32_t *row = p.ring + (size_t)b * p.L;
+#pragma unroll
+    for (int r = 0; r < kTR; ++r)
+        if ((r & 3) == q && rel0 + r < p.D + p.R && acc[r] != 0u) {
+            const int col = (int)((p.t0 + rel0 + r) % p.L);
+            if (gridDim.z == 1) row[col] += acc[r];
+            else atomicAdd(row + col, acc[r]);
+        }
+}
+
+// out[b][s] = the completed sample r = t0 - D + s (0 where r < 0: before the start of the stream); its ring column is cleared.
+__global__ void __launch_bounds__(256) dedisperse_emit_kernel(const StreamParams p) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (s >= p.R) return;
+    uint32_t *cell = p.ring + (size_t)b * p.L + (int)((p.t0 + s) % p.L);
+    p.out[(size_t)b * p.R + s] = (p.t0 + s >= p.D) ? *cell : 0u;
+    *cell = 0u;
+}
+
 }  // namespace chime_dd

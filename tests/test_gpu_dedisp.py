@@ -87,3 +87,45 @@ def test_chain_baseband_to_dedispersed_pulse(bf, orc):
     plain = orc.dedisperse(q, np.zeros_like(tab))
     assert want.max() > plain.max()
     plan.destroy()
+
+
+@pytest.mark.parametrize("dm,R,U", [(60.0, 24, 128), (500.0, 40, 128), (3.0, 16, 256)])
+def test_streaming_dedispersion_across_buffers(bf, orc, dm, R, U):
+    """Sweeps longer than one buffer ("a high nominal DM"): the stream of K buffers pushed one at a time
+    must give, sample for sample, the oracle's dedispersion of the concatenated stream.  DM 500 on this shortened band
+    (8 channels from 800 to 400 MHz) sweeps 9892 frames = 247 buffers of 40 frames; 12 buffers are pushed for DM 60."""
+    C = 8
+    freqs = np.linspace(800.0, 400.390625, C)
+    plan = bf.plan_create_ex(C, freq_mhz=freqs, upchan_len=U, n_time=R * 3 * U)
+    D = plan.dedisperse_stream_begin(dm)
+    delays, mx = orc.dedisp_delays(freqs, dm, U=U)
+    assert D == mx
+    K = int(np.ceil((D + 3 * R) / R)) + 1
+    rng = np.random.default_rng(int(dm))
+    # few beams carry data (the rest zero): the oracle's quadruple sum over 1024 beams x K R frames stays cheap
+    stream = np.zeros((C, K * R, 1024, 16), dtype=np.uint8)
+    bsel = [0, 5, 513, 1023]
+    stream[:, :, bsel, :] = rng.integers(0, 256, size=(C, K * R, len(bsel), 16), dtype=np.uint8)
+    want = orc.dedisperse(stream[:, :, bsel, :], delays)            # [4][K R - D]
+    got = np.zeros((1024, K * R), dtype=np.int64)
+    for k in range(K):
+        out, first = plan.dedisperse_stream_push(torch.from_numpy(stream[:, k * R:(k + 1) * R].copy()).cuda())
+        assert first == k * R - D
+        o = out.cpu().numpy().astype(np.int64)
+        for s in range(R):
+            r = first + s
+            if r >= 0:
+                got[:, r] = o[:, s]
+            else:
+                assert not o[:, s].any()
+    n = K * R - D - R       # samples completed by the pushes so far: r < K R - D, minus nothing; compare what both have
+    n = min(want.shape[1], (K - 0) * R - D)
+    assert n > R
+    assert np.array_equal(got[bsel, :n], want[:, :n])
+    assert not got[[1, 2, 700], :n].any()
+    # a second stream on the same plan starts clean
+    plan.dedisperse_stream_begin(dm / 2)
+    out, first = plan.dedisperse_stream_push(torch.from_numpy(stream[:, :R].copy()).cuda())
+    d2, mx2 = orc.dedisp_delays(freqs, dm / 2, U=U)
+    assert first == -mx2
+    plan.destroy()
