@@ -322,6 +322,9 @@ def dedisperse_beams(beams_u8, freq_mhz, dm, upchan_len=128, f_ref_mhz=0.0, stre
         raise ChimeBfError(f"dedisperse_beams: the DM {dm} sweep is longer than the {R}-frame buffer")
     out = torch.empty((nb, n_out), dtype=torch.int32, device=beams_u8.device)
     scratch = torch.empty(C * 16, dtype=torch.int32, device=beams_u8.device)
+    if stream is not None and not isinstance(stream, int):      # the kernel runs on `stream`: keep the caching allocator
+        out.record_stream(stream)                               # from re-using these blocks before it has finished
+        scratch.record_stream(stream)
     rc = load_library().chime_bf_dedisperse_beams(_stream_ptr(stream), beams_u8.data_ptr(), C, f.ctypes.data, R, nb,
                                                   upchan_len, float(dm), float(f_ref_mhz), scratch.data_ptr(),
                                                   out.data_ptr(), n_out)

@@ -331,6 +331,11 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         set_err("execute: null argument");
         return CHIME_BF_E_INVALID_ARG;
     }
+    int cur_dev = -1;
+    if (cudaGetDevice(&cur_dev) != cudaSuccess || cur_dev != pl->device) {
+        set_err("execute: the plan belongs to device %d, the current device is %d", pl->device, cur_dev);
+        return CHIME_BF_E_INVALID_ARG;
+    }
     if (((uintptr_t)in & 15) || ((uintptr_t)out_u8 & 15) || ((uintptr_t)out_f32 & 15)) {
         set_err("execute: buffers must be 16-byte aligned");
         return CHIME_BF_E_ALIGNMENT;
@@ -463,6 +468,12 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
         return nullptr;
     }
     if (!p.ew_angles_deg) { set_err("plan_create: ew_angles is NULL"); return nullptr; }
+    if (p.ns_sin_theta)
+        for (int m = 0; m < 256; ++m)
+            if (!(p.ns_sin_theta[m] >= -1.0 && p.ns_sin_theta[m] <= 1.0)) {
+                set_err("plan_create: ns_sin_theta[%d] outside [-1, 1]", m);
+                return nullptr;
+            }
     if ((long long)p.n_coarse * (p.n_time / (3 * p.upchan_len)) * 4 > 2147483647LL) {
         set_err("plan_create: grid too large");
         return nullptr;

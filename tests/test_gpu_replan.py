@@ -93,3 +93,20 @@ def test_update_tables_match_oracle_and_fresh_plan(bf, orc, NP, U):
     with pytest.raises(bf.ChimeBfError):
         plan.update_pointings(ns_sin_theta=np.full(256, 1.5))
     plan.destroy()
+
+
+def test_repointing_the_ew_beams_is_cheap_at_full_band(bf):
+    """Tracking E-W beams: on the tensor-core path a re-pointing uploads 32 bytes per channel (the E-W phase
+    steps), not the folded weight tables: well under a millisecond of stream time for all 1024 channels."""
+    import time
+    plan = bf.plan_create_ex(1024, n_time=384)
+    torch.cuda.synchronize()
+    plan.update_ew_angles((-0.5, -0.1, 0.3, 0.7))
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for k in range(20):
+        plan.update_ew_angles((-0.5 + 0.01 * k, -0.1, 0.3, 0.7))
+    torch.cuda.synchronize()
+    dt = (time.perf_counter() - t0) / 20
+    assert dt < 1e-3, dt
+    plan.destroy()
