@@ -246,16 +246,14 @@ __device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned cha
 }
 
 // ---- accumulator drain: one digit pass (64 s32 columns of this thread's lane) folded into 64 fp32 partial sums ------
-// Every accumulator column STARTS from the bit pattern of 1.5 * 2^23 (written by the previous drain), so what comes out
-// is already the float M + a (|a| < 2^22, exact): y = a2 + a1 / 256 + a0 / 65536 in units of the top digit costs one
-// instruction per value and pass.  Column n = 32 variant + 16 set + u'.
+// |a| < 2^22 (K 512 x 128 x 64), so the integer a + 0x4B400000 IS the bit pattern of the float M + a, M = 1.5 * 2^23
+// (exact): the conversion is one integer add (ALU pipe), and y = a2 + a1 / 256 + a0 / 65536 in units of the top digit
+// costs one more FP32 instruction per value and pass.  Column 32 part + j (part 0 = real, 1 = imaginary, j = 16 set +
+// u') goes to y[2 j + part], so that (re, im) pairs and the 16-byte groups the sender stores sit in consecutive
+// registers.  The hand-back of the slot is the critical path of the whole pipeline (two 64-column slots rotate under
+// three digit passes), so it happens as soon as the columns are in registers, BEFORE the arithmetic.
 constexpr uint32_t kMagicBits = 0x4B400000u;               // 1.5 * 2^23 = 12582912
 constexpr float kMagicSum = 12582912.0f + 49152.0f + 192.0f;   // M (1 + 2^-8 + 2^-16), an exact integer < 2^24
-
-__device__ __forceinline__ void tmem_fill16(uint32_t taddr, uint32_t v) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1};"
-                 :: "r"(taddr), "r"(v) : "memory");
-}
 
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t *v) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -268,30 +266,28 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t *v) {
                  : "r"(taddr) : "memory");
 }
 
-// One digit pass of this thread's 64 columns folded into y; the columns are refilled with the magic constant for the
-// slot's next pass.  Every accumulator column starts from the bit pattern of M = 1.5 * 2^23, so what is loaded is
-// already the float M + a (|a| < 2^22, exact): y = a2 + a1 / 256 + a0 / 65536 in units of the top digit costs one
-// instruction per value and pass.  Column 32 part + j (part 0 = real, 1 = imaginary, j = 16 set + u') goes to
-// y[2 j + part], so that (re, im) pairs and the 16-byte groups the sender stores sit in consecutive registers.
+__device__ __forceinline__ void slot_release(const uint32_t bar_empty, const int lane) {
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_empty);   // the slot is in registers: hand it back to the issuer
+}
+
 template <int P>
-__device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64]) {
+__device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64], const uint32_t bar_empty, const int lane) {
+    constexpr float kS = P == 1 ? 1.0f / 256.0f : 1.0f / 65536.0f;
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {   // 16 columns at a time: c = 2 part + set
-        uint32_t h[16];
-        tmem_ld16(tslot + 16 * c, h);
+    for (int hf = 0; hf < 2; ++hf) {   // hf = part: 32 columns at a time
+        uint32_t h[32];
+        tmem_ld32(tslot + 32 * hf, h);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        tmem_fill16(tslot + 16 * c, kMagicBits);
-        const int part = c >> 1;
+        if (hf == 1) slot_release(bar_empty, lane);
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-            const int j = 16 * (c & 1) + i;
-            const float f = __uint_as_float(h[i]);
-            if constexpr (P == 0) y[2 * j + part] = f - kMagicSum;
-            else if constexpr (P == 1) y[2 * j + part] = fmaf(f, 1.0f / 256.0f, y[2 * j + part]);
-            else y[2 * j + part] = fmaf(f, 1.0f / 65536.0f, y[2 * j + part]);
+        for (int j = 0; j < 32; ++j) {
+            const float f = __uint_as_float(h[j] + kMagicBits);
+            if constexpr (P == 0) y[2 * j + hf] = f - kMagicSum;
+            else y[2 * j + hf] = fmaf(f, kS, y[2 * j + hf]);
         }
     }
-    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
 // One tile on the drain side (the two drain groups take alternate tiles, so that one group's DSMEM stores overlap the
@@ -314,12 +310,9 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, con
         n_use1 += slot;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t tslot = tlane + kWCols + 64 * slot;
-        if (p == 0) drain_pass<0>(tslot, y);
-        else if (p == 1) drain_pass<1>(tslot, y);
-        else drain_pass<2>(tslot, y);
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_empty0 + 8 * slot);   // the slot is in registers: hand it back to the issuer
+        if (p == 0) drain_pass<0>(tslot, y, bar_empty0 + 8 * slot, lane);
+        else if (p == 1) drain_pass<1>(tslot, y, bar_empty0 + 8 * slot, lane);
+        else drain_pass<2>(tslot, y, bar_empty0 + 8 * slot, lane);
     }
     if (tt >= 2) {   // A_rho = E + O'/sqrt2 (set 0), A_{rho+4} = E - O'/sqrt2 (set 1)
         constexpr float s = 0.70710678118654752440f;
@@ -437,7 +430,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                             const uint32_t d = tb + kWCols + 64 * myslot;
                             uint32_t a = tb + 128 * p;
                             uint64_t bd = bd0;
-                            umma_i8_ts<true>(d, a, bd, idesc);
+                            umma_i8_ts<false>(d, a, bd, idesc);   // the first K step of a pass overwrites the slot
 #pragma unroll 1
                             for (int k = 1; k < 16; ++k) {   // rolled: the issuers run on 32 registers
                                 a += 8;
@@ -541,16 +534,9 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
         const uint32_t accf = BAR(B_ACC_FULL + 2 * g), acce = BAR(B_ACC_EMPTY + 2 * g);
         uint32_t n_use0 = 0, n_use1 = 0;
         uint32_t tau = 0;
-        if (g == 0) {   // both accumulator slots start from the magic constant: group 0's "drain number 0" of each slot
-#pragma unroll
-            for (int c = 0; c < 8; ++c) tmem_fill16(tlane + kWCols + 16 * c, kMagicBits);
-            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) {
-                mbar_arrive(acce);
-                mbar_arrive(acce + 8);
-            }
+        if (g == 0 && lane == 0) {   // both accumulator slots start empty: group 0's "drain number 0" of each slot
+            mbar_arrive(acce);
+            mbar_arrive(acce + 8);
         }
         ITEM_LOOP
             for (int pol = 0; pol < 2; ++pol) {
