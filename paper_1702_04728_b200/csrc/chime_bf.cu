@@ -256,6 +256,10 @@ bool build_tables(chime_bf_plan *pl) {
             tw128[k] = make_float2((float)std::cos(a), (float)std::sin(a));
         }
         CUDA_TRY(cudaMemcpyToSymbol(chime4::c_tw128, tw128.data(), sizeof(float2) * 128));
+        std::vector<float2> twr(8 * 16);
+        for (int rho = 0; rho < 8; ++rho)
+            for (int u = 0; u < 16; ++u) twr[rho * 16 + u] = tw128[(rho * u) & 127];
+        CUDA_TRY(cudaMemcpyToSymbol(chime4::c_twr, twr.data(), sizeof(float2) * 128));
         CUDA_TRY(cudaFuncSetAttribute(chime4::umma_beamform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, chime4::kSmemBytes));
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(4 * 148);

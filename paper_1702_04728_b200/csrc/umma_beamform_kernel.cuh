@@ -41,7 +41,7 @@
 #include <stdint.h>
 
 #include "beamform_kernel.cuh"       // chime::beam_major_dst
-#include "int_butterflies.cuh"       // chime4::int_bfly4, c_tw128
+#include "int_butterflies.cuh"       // chime4::int_bfly4, c_twr
 #include "fft_regs.cuh"
 
 namespace chime4 {
@@ -109,12 +109,12 @@ __device__ __forceinline__ uint32_t mapa(uint32_t a, uint32_t rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
     return r;
 }
-// try_wait with a suspend-time hint: the hardware parks the warp until the phase completes (or the hint expires)
-// instead of letting it spin through the issue slots the working warps need.
+// try_wait parks the warp in hardware until the phase completes or a system time limit expires.  (With a suspend-time
+// hint ptxas adds a NANOSLEEP and a second phase check per poll: 1 % slower, measured.)
 __device__ __forceinline__ bool mbar_try(uint32_t a, uint32_t parity) {
     uint32_t ok;
-    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3; selp.u32 %0, 1, 0, p; }"
-                 : "=r"(ok) : "r"(a), "r"(parity), "r"(20000u) : "memory");
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(a), "r"(parity) : "memory");
     return ok != 0;
 }
 #ifdef CHIME_PROF
@@ -123,7 +123,7 @@ __device__ long long g_prof[148 * 4][24][12];
 #else
 #define PW(code, stmt) { stmt; }
 #endif
-// Waits for the phase of parity `parity` to complete.  A wait of ~2^20 polls (each up to 20 us) is a protocol bug:
+// Waits for the phase of parity `parity` to complete.  A wait of ~2^20 polls (seconds) is a protocol bug:
 // flag it and trap instead of hanging the GPU.
 __device__ __forceinline__ void mbar_timeout(int *status, int code, uint32_t info) {
     atomicCAS(status + code * 8 + (blockIdx.x & 7), 0, 1 | ((int)(threadIdx.x >> 5) << 8) | ((int)info << 16));
@@ -281,9 +281,13 @@ __device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64],
         tmem_ld32(tslot + 32 * hf, h);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
         if (hf == 1) slot_release(bar_empty, lane);
+#if defined(CHIME_SKIP) && (CHIME_SKIP & 4)
+        y[hf] = __uint_as_float(h[0] ^ h[31]);
+        if (lane > 32)
+#endif
 #pragma unroll
         for (int j = 0; j < 32; ++j) {
-            const float f = __uint_as_float(h[j] + kMagicBits);
+            const float f = __uint_as_float(h[j] + kMagicBits);   // (cvt.rn.f32.s32 instead: 5 % slower, measured)
             if constexpr (P == 0) y[2 * j + hf] = f - kMagicSum;
             else y[2 * j + hf] = fmaf(f, kS, y[2 * j + hf]);
         }
@@ -509,6 +513,9 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                             const uint32_t s = tau & 1;
                             PW(8, mbar_wait(BAR(B_BOP_EMPTY + s), ((tau >> 1) & 1) ^ 1, status, 8, tau);)
                             unsigned char *bop = smem + kOfsBop + s * kBopBytes;
+#if defined(CHIME_SKIP) && (CHIME_SKIP & 2)
+                            if (prm.n_time < 0)
+#endif
                             switch (tt) {
                                 case 0: prep_tile<0>(raw, bop, pw, lane); break;
                                 case 1: prep_tile<1>(raw, bop, pw, lane); break;
@@ -583,6 +590,9 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                         PW(10, mbar_wait(BAR(B_RECV_FULL + s), (tau >> 1) & 1, status, 10, tau);)
                         if (rw == 0 && lane == 0) mbar_expect_tx(BAR(B_RECV_FULL + s), kRecvBytes);   // arm the slot's next tile
                         unsigned char *slot = smem + kOfsRecv + s * kRecvBytes + lane * 16;
+#if defined(CHIME_SKIP) && (CHIME_SKIP & 1)
+                        if (prm.n_time < 0)
+#endif
                         {   // ---- phase 1: (beam, u' pair = rw), both residues
                             unsigned char *base = slot + rw * 512;
 #pragma unroll
@@ -603,11 +613,17 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                                         za = __ffma2_rn(make_float2(za.y, za.x), by, ta);
                                         zb = __ffma2_rn(make_float2(zb.y, zb.x), by, tb2);
                                     }
-                                    *reinterpret_cast<float4 *>(base + ((e * 2 + res) * 8) * 512) = make_float4(za.x, za.y, zb.x, zb.y);
+                                    // two 8-byte stores: a 16-byte one costs four register moves (za, zb are not neighbours)
+                                    const uint32_t oa = smem_u32(base + ((e * 2 + res) * 8) * 512);
+                                    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(oa), "f"(za.x), "f"(za.y) : "memory");
+                                    asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" :: "r"(oa), "f"(zb.x), "f"(zb.y) : "memory");
                                 }
                             }
                         }
                         bar_sync_named(1, 256);
+#if defined(CHIME_SKIP) && (CHIME_SKIP & 1)
+                        if (prm.n_time < 0)
+#endif
                         {   // ---- phase 2: (beam, residue = res2, E-W beam = e2)
                             const unsigned char *base = slot + ((e2 * 2 + res2) * 8) * 512;
                             float2 a[16];
@@ -621,7 +637,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                             const int tt = t & 3;
                             const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
 #pragma unroll
-                            for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_tw128[(rho * u) & 127]);
+                            for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr[rho][u]);
                             fft_dif<16>(a);
 #pragma unroll
                             for (int i = 0; i < 16; ++i) {
