@@ -266,21 +266,38 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t *v) {
                  : "r"(taddr) : "memory");
 }
 
-__device__ __forceinline__ void slot_release(const uint32_t bar_empty, const int lane) {
+#ifdef CHIME_PROF
+__device__ __forceinline__ volatile long long *prof_trel() {
+    __shared__ long long s_trel[2][4];
+    return &s_trel[0][0];
+}
+#endif
+// Hand-back of an accumulator slot: a NAMED barrier (id 2 + slot) that the 4 warps of the draining group arrive on
+// without waiting and the slot's issuer waits on -- measured 240 cycles from arrive to the issuer's next instruction
+// through an mbarrier + try_wait, a fraction of that through bar.arrive / bar.sync.
+constexpr int kSlotBarThreads = 4 * 32 + 32;
+__device__ __forceinline__ void slot_release(const uint32_t slot, const int lane) {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncwarp();
-    if (lane == 0) mbar_arrive(bar_empty);   // the slot is in registers: hand it back to the issuer
+#ifdef CHIME_PROF
+    if (lane == 0) prof_trel()[4 * slot + ((threadIdx.x >> 5) & 3)] = clock64();
+#endif
+    asm volatile("bar.arrive %0, %1;" :: "r"(2 + slot), "n"(kSlotBarThreads) : "memory");
 }
 
 template <int P>
-__device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64], const uint32_t bar_empty, const int lane) {
+__device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64], const uint32_t slot, const int lane, long long *t_rel = nullptr) {
     constexpr float kS = P == 1 ? 1.0f / 256.0f : 1.0f / 65536.0f;
 #pragma unroll
     for (int hf = 0; hf < 2; ++hf) {   // hf = part: 32 columns at a time
         uint32_t h[32];
         tmem_ld32(tslot + 32 * hf, h);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        if (hf == 1) slot_release(bar_empty, lane);
+        if (hf == 1) {
+            slot_release(slot, lane);
+#ifdef CHIME_PROF
+            *t_rel = clock64();
+#endif
+        }
 #if defined(CHIME_SKIP) && (CHIME_SKIP & 4)
         y[hf] = __uint_as_float(h[0] ^ h[31]);
         if (lane > 32)
@@ -300,7 +317,7 @@ __device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64],
 // folded into y and the slot handed back at once.  Odd-residue tiles (tt >= 2) combine E and O' here; the rest of the
 // time transform (twiddle, FFT-16) is linear and runs AFTER the E-W sum on the receiving side.
 // Receive slot layout: [cyl 4][res 2][u' pair 8][beam 32] x {re, im, re, im}.
-__device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, const uint32_t bar_full0, const uint32_t bar_empty0,
+__device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, const uint32_t bar_full0,
                                          uint32_t &n_use0, uint32_t &n_use1, const uint32_t tau, const uint32_t rslot, const uint32_t rbar,
                                          const int cyl, const int lane, const uint32_t slot_free_bar,
                                          const uint32_t sf_parity, int *status, long long *prof_w) {
@@ -314,9 +331,21 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, con
         n_use1 += slot;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t tslot = tlane + kWCols + 64 * slot;
-        if (p == 0) drain_pass<0>(tslot, y, bar_empty0 + 8 * slot, lane);
-        else if (p == 1) drain_pass<1>(tslot, y, bar_empty0 + 8 * slot, lane);
-        else drain_pass<2>(tslot, y, bar_empty0 + 8 * slot, lane);
+#ifdef CHIME_PROF
+        const long long _t0 = clock64();
+#endif
+#ifdef CHIME_PROF
+        long long _t1 = 0;
+        if (p == 0) drain_pass<0>(tslot, y, slot, lane, &_t1);
+        else if (p == 1) drain_pass<1>(tslot, y, slot, lane, &_t1);
+        else drain_pass<2>(tslot, y, slot, lane, &_t1);
+        prof_w[6] += _t1 - _t0;
+        prof_w[7] += clock64() - _t1;
+#else
+        if (p == 0) drain_pass<0>(tslot, y, slot, lane);
+        else if (p == 1) drain_pass<1>(tslot, y, slot, lane);
+        else drain_pass<2>(tslot, y, slot, lane);
+#endif
     }
     if (tt >= 2) {   // A_rho = E + O'/sqrt2 (set 0), A_{rho+4} = E - O'/sqrt2 (set 1)
         constexpr float s = 0.70710678118654752440f;
@@ -362,7 +391,6 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
         for (int i = 0; i < 8; ++i) mbar_init(BAR(B_SLOT_FREE + i), 8);
         for (int i = 0; i < 4; ++i) {
             mbar_init(BAR(B_ACC_FULL + i), 1);    // accumulator slot, per drain group: one commit per digit pass
-            mbar_init(BAR(B_ACC_EMPTY + i), 4);   // ... drained by the 4 warps of the group
         }
         mbar_init(BAR(B_W_FREE), 2);
         mbar_init(BAR(B_W_READY), 4);
@@ -412,8 +440,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
         // order; the issuer waits for the drain of the slot's PREVIOUS use, whichever group that was.
         const uint32_t myslot = warp;
         uint32_t tau = 0, seg = 0;
-        uint32_t n_use0 = 1, n_use1 = 0;   // drains of my slot requested so far, per group (group 0's initial fill counts)
-        int prev_g = 0;                    // group that drains (fills) my slot before my next pass
+        uint32_t n_mine = 0;               // passes issued to my slot
         ITEM_LOOP
             for (int pol = 0; pol < 2; ++pol) {
                 PW(1, mbar_wait(BAR(B_W_READY), seg & 1, status, 1, seg);)
@@ -428,8 +455,22 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                         const uint32_t pi = 3 * tau + p;
                         if ((pi & 1) != myslot) continue;
                         const int g = tau & 1;
-                        PW(3, mbar_wait(BAR(B_ACC_EMPTY + 2 * prev_g + myslot), ((prev_g ? n_use1 : n_use0) - 1) & 1, status, 3, tau);)
+#ifdef CHIME_PROF
+                        const long long _tw = clock64();
+#endif
+                        // the drain of my slot's previous pass (whichever group that was) has its columns in registers
+                        if (n_mine > 0) { PW(3, asm volatile("bar.sync %0, %1;" :: "r"(2 + myslot), "n"(kSlotBarThreads) : "memory");) }
+                        ++n_mine;
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#ifdef CHIME_PROF
+                        const long long _t0 = clock64();
+                        {
+                            volatile long long *tr = prof_trel() + 4 * myslot;
+                            long long m = tr[0];
+                            for (int i = 1; i < 4; ++i) m = tr[i] > m ? tr[i] : m;
+                            if (m > _tw && _t0 > m) { prof_w[5] += _t0 - m; prof_w[8] += 1; }   // the release came while I was waiting
+                        }
+#endif
                         if (elect_one()) {
                             const uint32_t d = tb + kWCols + 64 * myslot;
                             uint32_t a = tb + 128 * p;
@@ -444,9 +485,9 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                             umma_commit(BAR(B_ACC_FULL + 2 * g + myslot));
                         }
                         __syncwarp();
-                        n_use0 += 1 - g;
-                        n_use1 += g;
-                        prev_g = g;
+#ifdef CHIME_PROF
+                        prof_w[4] += clock64() - _t0;
+#endif
                     }
                     if (elect_one()) umma_commit(BAR(B_BOP_EMPTY + s));   // both issuers: the B tile is free when all 3 passes are done
                     __syncwarp();
@@ -538,20 +579,16 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
         const uint32_t rslot = mapa(smem_u32(smem + kOfsRecv) + g * kRecvBytes, q);
         const uint32_t rfull = mapa(BAR(B_RECV_FULL + g), q);
         const uint32_t sfree = BAR(B_SLOT_FREE + 2 * q + g);
-        const uint32_t accf = BAR(B_ACC_FULL + 2 * g), acce = BAR(B_ACC_EMPTY + 2 * g);
+        const uint32_t accf = BAR(B_ACC_FULL + 2 * g);
         uint32_t n_use0 = 0, n_use1 = 0;
         uint32_t tau = 0;
-        if (g == 0 && lane == 0) {   // both accumulator slots start empty: group 0's "drain number 0" of each slot
-            mbar_arrive(acce);
-            mbar_arrive(acce + 8);
-        }
         ITEM_LOOP
             for (int pol = 0; pol < 2; ++pol) {
                 const int ntiles = nf * 12;
 #pragma unroll 1
                 for (int t = 0; t < ntiles; ++t, ++tau) {
                     if ((int)(tau & 1) != g) continue;
-                    epi_tile(t & 3, tlane, accf, acce, n_use0, n_use1, tau, rslot, rfull, rank, lane, sfree, ((tau >> 1) & 1) ^ 1, status, prof_w);
+                    epi_tile(t & 3, tlane, accf, n_use0, n_use1, tau, rslot, rfull, rank, lane, sfree, ((tau >> 1) & 1) ^ 1, status, prof_w);
                 }
             }
         }
@@ -633,6 +670,24 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                                 a[2 * k] = make_float2(v.x, v.y);
                                 a[2 * k + 1] = make_float2(v.z, v.w);
                             }
+                            // The slot is in registers: hand it back to the four senders BEFORE the arithmetic.  The
+                            // arrive is made to depend on one word of every load, so that it cannot be issued while a
+                            // load is still in flight.
+                            {
+                                uint32_t dep;
+                                asm volatile("{ .reg .b32 t0, t1;\n or.b32 t0, %1, %2;\n or.b32 t1, %3, %4;\n or.b32 t0, t0, t1;\n"
+                                             " or.b32 t1, %5, %6;\n or.b32 t0, t0, t1;\n or.b32 t1, %7, %8;\n or.b32 t0, t0, t1;\n"
+                                             " or.b32 %0, t0, 1; }"
+                                             : "=r"(dep)
+                                             : "r"(__float_as_uint(a[1].y)), "r"(__float_as_uint(a[3].y)), "r"(__float_as_uint(a[5].y)),
+                                               "r"(__float_as_uint(a[7].y)), "r"(__float_as_uint(a[9].y)), "r"(__float_as_uint(a[11].y)),
+                                               "r"(__float_as_uint(a[13].y)), "r"(__float_as_uint(a[15].y)));
+                                dep = __reduce_or_sync(0xffffffffu, dep);   // every lane's loads
+                                if (lane == 0 && dep != 0) {
+#pragma unroll
+                                    for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc] + 8 * s);
+                                }
+                            }
                             // residue of (tile type, column set): {0,4}, {2,6}, {1,5}, {3,7}
                             const int tt = t & 3;
                             const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
@@ -644,11 +699,6 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                                 const int g = (bitrev(i, 4) + 8) & 15;
                                 acc[g] = fmaf(a[i].x, a[i].x, fmaf(a[i].y, a[i].y, acc[g]));
                             }
-                        }
-                        __syncwarp();
-                        if (lane == 0) {
-#pragma unroll
-                            for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc] + 8 * s);
                         }
                     }
                     // ---- frame end: a9 sum of the two residue halves (+ pol 0), normalise, a10 quantise, 16-byte store per beam
