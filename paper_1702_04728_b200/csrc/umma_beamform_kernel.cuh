@@ -131,6 +131,17 @@ __device__ __forceinline__ void mbar_timeout(int *status, int code, uint32_t inf
     for (long long t1 = clock64(); clock64() - t1 < 1500000000ll;) {}
     __trap();
 }
+// Latency-critical waits: test_wait does not park the warp, so the phase flip is seen within one poll.
+__device__ __forceinline__ void mbar_spin(uint32_t a, uint32_t parity, int *status, int code, uint32_t info = 0) {
+    uint32_t n = 0;
+    while (true) {
+        uint32_t ok;
+        asm volatile("{ .reg .pred p; mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        if (ok) break;
+        if (++n > (1u << 26)) mbar_timeout(status, code, info);
+    }
+}
 __device__ __forceinline__ void mbar_wait(uint32_t a, uint32_t parity, int *status, int code, uint32_t info = 0) {
     uint32_t n = 0;
     while (!mbar_try(a, parity))
@@ -276,6 +287,7 @@ __device__ __forceinline__ volatile long long *prof_trel() {
 // without waiting and the slot's issuer waits on -- measured 240 cycles from arrive to the issuer's next instruction
 // through an mbarrier + try_wait, a fraction of that through bar.arrive / bar.sync.
 constexpr int kSlotBarThreads = 4 * 32 + 32;
+constexpr int kBopBarThreads = 4 * 32 + 2 * 32;   // B tile ready (id 4 + slot): 4 preparing warps arrive, both issuers wait
 __device__ __forceinline__ void slot_release(const uint32_t slot, const int lane) {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
 #ifdef CHIME_PROF
@@ -326,7 +338,11 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, con
     for (int p = 0; p < 3; ++p) {
         const uint32_t slot = (tau + p) & 1;     // = (3 tau + p) & 1
         const uint32_t use = slot ? n_use1 : n_use0;
+#ifdef CHIME_SPINFULL
+        PW(9, mbar_spin(bar_full0 + 8 * slot, use & 1, status, 9, tau);)
+#else
         PW(9, mbar_wait(bar_full0 + 8 * slot, use & 1, status, 9, tau);)
+#endif
         n_use0 += 1 - slot;
         n_use1 += slot;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -448,7 +464,8 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                 const int ntiles = nf * 12;
                 for (int t = 0; t < ntiles; ++t, ++tau) {
                     const uint32_t s = tau & 1, ph = (tau >> 1) & 1;
-                    PW(2, mbar_wait(BAR(B_BOP_FULL + s), ph, status, 2, tau);)
+                    (void)ph;
+                    PW(2, asm volatile("bar.sync %0, %1;" :: "r"(4 + s), "n"(kBopBarThreads) : "memory");)   // the B tile is written
                     const uint64_t bd0 = make_desc(smem_u32(smem + kOfsBop) + s * kBopBytes, 1024, 128);
 #pragma unroll 1
                     for (uint32_t p = 0; p < 3; ++p) {
@@ -564,8 +581,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
                                 default: prep_tile<3>(raw, bop, pw, lane); break;
                             }
                             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes -> tensor-core reads
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(BAR(B_BOP_FULL + s));
+                            asm volatile("bar.arrive %0, %1;" :: "r"(4 + s), "n"(kBopBarThreads) : "memory");   // named barrier: see slot_release
                         }
                         __syncwarp();
                         if (lane == 0) mbar_arrive(BAR(B_RAW_EMPTY + b));
