@@ -246,6 +246,37 @@ bool build_umma_weights(chime_bf_plan *pl, cudaStream_t st) {
     return true;
 }
 
+// The packed baseband [rows = C * T][2048 bytes] as a 2-D tensor map for the kernel's TMA loads: box 128 bytes x 128 rows
+// (one half of a (pol, cylinder) block), 128-byte swizzle.  The encoder lives in the driver; it is fetched through the
+// runtime so that the library does not link libcuda.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+bool encode_input_map(CUtensorMap *map, const uint8_t *in, size_t rows) {
+    static EncodeTiledFn fn = nullptr;
+    if (fn == nullptr) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || p == nullptr) {
+            set_err("execute: cuTensorMapEncodeTiled is not available in this driver");
+            return false;
+        }
+        fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    const cuuint64_t dims[2] = {2048, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {2048};
+    const cuuint32_t box[2] = {128, 128};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t *>(in), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_err("execute: cuTensorMapEncodeTiled failed (%d)", (int)r);
+        return false;
+    }
+    return true;
+}
+
 bool build_tables(chime_bf_plan *pl) {
     const int NP = pl->NP, U = pl->U;
     if (!build_index_tables(pl, nullptr)) return false;
@@ -396,7 +427,9 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         up.chunk_frames = chunk;
         const long long n_items = (long long)n_chan * ((n_fr + chunk - 1) / chunk) * 2;
         const int n_cl = (int)std::min<long long>(n_items, pl->max_clusters);
-        chime4::umma_beamform_kernel<<<4 * n_cl, chime4::kThreads, chime4::kSmemBytes, st>>>(up);
+        CUtensorMap tmap;
+        if (!encode_input_map(&tmap, in, (size_t)pl->C * pl->T)) return CHIME_BF_E_CUDA;
+        chime4::umma_beamform_kernel<<<4 * n_cl, chime4::kThreads, chime4::kSmemBytes, st>>>(up, tmap);
         const cudaError_t e4 = cudaGetLastError();
         if (e4 != cudaSuccess) {
             set_err("kernel launch failed: %s", cudaGetErrorString(e4));

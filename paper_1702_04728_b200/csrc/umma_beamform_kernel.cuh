@@ -37,6 +37,7 @@
 //   warps 16-23   receive side: E-W Horner, detect, accumulate; item epilogue (normalise, quantise, store)
 // All hand-overs are mbarriers (local, or remote through mapa for the two cluster-level ones).
 #pragma once
+#include <cuda.h>            // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -386,7 +387,10 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, con
         }
 }
 
-__global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_beamform_kernel(const Params prm) {
+// tmap: the packed baseband as a 2-D byte tensor [C * T rows][2048], box 128 bytes x 128 rows, 128-byte swizzle (the
+// layout prep_tile reads: 16-byte chunk index ^ (row & 7) inside every 128-byte row).
+__global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1)
+umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     uint32_t rank;
@@ -398,7 +402,7 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
 
     if (tid == 0) {
         for (int s = 0; s < 2; ++s) {
-            mbar_init(BAR(B_RAW_FULL + s), 64);
+            mbar_init(BAR(B_RAW_FULL + s), 1);    // one expect_tx arrive; the TMA reports the bytes
             mbar_init(BAR(B_RAW_EMPTY + s), 4);
             mbar_init(BAR(B_BOP_FULL + s), 4);
             mbar_init(BAR(B_BOP_EMPTY + s), 2);
@@ -515,27 +519,31 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1) umma_be
             }
         }
     } else if (warp < 4) {
-        // ============================== raw-block stagers ==============================
-        const int st = tid - 64;
-        uint32_t beta = 0;
-        ITEM_LOOP
-            for (int pol = 0; pol < 2; ++pol)
-                for (int fr = 0; fr < nf; ++fr)
-                    for (int blk = 0; blk < 3; ++blk, ++beta) {
-                        const uint32_t b = beta & 1;
-                        PW(4, mbar_wait(BAR(B_RAW_EMPTY + b), ((beta >> 1) & 1) ^ 1, status, 4, beta);)
-                        const size_t t0 = (size_t)((fr0 + fr) * 3 + blk) * 128;
-                        const uint8_t *src = prm.in + ((size_t)c * prm.n_time + t0) * 2048 + pol * 1024 + rank * 256;
-                        const uint32_t dst = smem_u32(smem + kOfsRaw) + b * kRawBytes;
-                        for (int idx = st; idx < 2048; idx += 64) {
-                            const int t = idx >> 4, j = idx & 15;
-                            const uint32_t d = dst + (j >> 3) * 16384 + t * 128 + (((j & 7) ^ (t & 7)) << 4);
-                            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(src + (size_t)t * 2048 + j * 16) : "memory");
+        // ============================== raw-block stager: one lane, two TMA loads per block ==============================
+        // A block = 128 time samples x 256 bytes of (pol, cylinder): two boxes of 128 rows x 128 bytes (feeds 0-127,
+        // 128-255), each 16 KiB, swizzled by the copy engine.
+        if (warp == 2) {
+            uint32_t beta = 0;
+            ITEM_LOOP
+                for (int pol = 0; pol < 2; ++pol)
+                    for (int fr = 0; fr < nf; ++fr)
+                        for (int blk = 0; blk < 3; ++blk, ++beta) {
+                            const uint32_t b = beta & 1;
+                            PW(4, mbar_wait(BAR(B_RAW_EMPTY + b), ((beta >> 1) & 1) ^ 1, status, 4, beta);)
+                            if (elect_one()) {
+                                const int row = c * prm.n_time + ((fr0 + fr) * 3 + blk) * 128;
+                                const int col = pol * 1024 + (int)rank * 256;
+                                const uint32_t dst = smem_u32(smem + kOfsRaw) + b * kRawBytes, bar = BAR(B_RAW_FULL + b);
+                                mbar_expect_tx(bar, kRawBytes);
+                                asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                                             :: "r"(dst), "l"(&tmap), "r"(col), "r"(row), "r"(bar) : "memory");
+                                asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                                             :: "r"(dst + 16384), "l"(&tmap), "r"(col + 128), "r"(row), "r"(bar) : "memory");
+                            }
+                            __syncwarp();
                         }
-                        asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" :: "r"(BAR(B_RAW_FULL + b)) : "memory");
-                    }
+            }
         }
-        asm volatile("cp.async.wait_all;" ::: "memory");
     } else if (warp < 8) {
         // ============================== operand preparation + weight loads ==============================
         const int pw = warp - 4;   // = TMEM lane quarter for the weight loads (warp % 4)
