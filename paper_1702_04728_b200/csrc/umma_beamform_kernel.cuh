@@ -4,7 +4,7 @@
 // integration and quantisation (a8-a10) run on the FP32 pipe around it.  upchan_len = 128, any zero_pad (the padding
 // factor only changes the weights).  PAPER.md:51-53 (the three kernels), :59-61 (N-S transform), :84-86 (up-channelise).
 //
-// Mathematics (DESIGN.md 5.7).  All operators before |.|^2 are linear and act on different axes, so they commute:
+// Mathematics (DESIGN.md 5.1).  All operators before |.|^2 are linear and act on different axes, so they commute:
 //   1. time, first stage, on the raw 4-bit integers (exact, packed four feeds per register): with t = u' + 16 k,
 //        S[8 q' + rho] = sum_{u'<16} W_16^{q'u'} W_128^{rho u'} A_rho[u'],   A_rho[u'] = sum_{k<8} x[u' + 16 k] W_8^{rho k}
 //      A_rho = E_rho + W_8^rho O_rho (even / odd taps).  Even rho: A_rho is a Gaussian integer, |re|,|im| <= 64.
@@ -12,30 +12,32 @@
 //      go through the GEMM separately and are combined in fp32.
 //   2. N-S (+ gains, + bin selection): Y[m] = sum_n (g[n] W_NP^{J[m] n}) a[n] for a = A_rho[u'] (or E, O'): one row of
 //      a [256 beams x 2] x [256 feeds x 2] real matrix per (channel, pol, cylinder), the same for every column a.
-//      Weights = round(S_c * value) as 16-bit integers split into two signed 8-bit digits (256 hi + lo) that stay
-//      resident in TENSOR MEMORY (128 lanes = 128 beams, 2 x 128 columns = K 512 x 2 digits); the data columns are
-//      unsigned bytes (value + bias) in shared memory; two s32 accumulators (hi, lo) per output, recombined exactly in
-//      fp32 (256 hi + lo, bias * rowsum removed in the integer domain).  Real and imaginary outputs of a beam come
+//      Weights = round(S_c * value) as 24-bit integers split into THREE balanced signed 8-bit digits (16 bits fail the
+//      1e-4 parity bar on configs[0]) that stay resident in TENSOR MEMORY (128 lanes = 128 beams,
+//      3 x 128 columns = K 512 x 3 digits); the data columns are signed bytes in shared memory; one s32 accumulator
+//      pass per digit, recombined in fp32 as a2 + a1 / 256 + a0 / 65536.  Real and imaginary outputs of a beam come
 //      from the SAME weight row [Wr | -Wi] applied to two variants of the data column, [re | im] and [im | -re], so
 //      both land in the same TMEM lane (= thread) in different columns.
-//   3. time, second stage, per cylinder (thread <-> beam, 16 values in registers): twiddle W_128^{rho u'}, FFT-16.
-//   4. E-W: Z_e = sum_cyl beta_e^cyl S_cyl (Horner), after an all-to-all by beam quarter over DSMEM: CTA r of the
+//   3. E-W: Z_e = sum_cyl beta_e^cyl S_cyl (Horner), after an all-to-all by beam quarter over DSMEM: CTA r of the
 //      cluster owns cylinder r on the way in and beams 32 r .. 32 r + 31 of the tile on the way out.
+//   4. time, second stage, per (beam, residue, E-W beam): twiddle W_128^{rho u'}, FFT-16 over u'.
 //   5. |Z|^2, sum over the 8 bins of a fine channel (= over rho), the 2 polarisations and the 3 blocks; quantise.
 //
-// Work decomposition: item = (channel, tile of 128 beams, chunk of up to 4 output frames), handed round-robin to the
-// clusters of a persistent grid.  Within an item the cluster runs polarisation 0 then 1 (weights reloaded in between)
-// and keeps the 4 frames' intensities in registers.  Per (block of 128 samples, pol) a CTA stages the raw 32 KiB of its
-// cylinder once (cp.async, XOR-swizzled) and makes 4 tiles from it (residue pairs {0,4}, {2,6}, {1,5}, {3,7}), each
-// a 128 x 64 x 512 x 2-digit GEMM (32 tcgen05.mma of K = 32) into one of two TMEM accumulator stages.
+// Work decomposition: item = (channel, tile of 128 beams, chunk of up to 16 output frames), handed round-robin to the
+// clusters of a persistent grid.  Within an item the cluster runs polarisation 0 then 1 (weights reloaded in between);
+// the polarisation-0 sums of a frame wait in a per-CTA scratch (L2).  Per (block of 128 samples, pol) a CTA stages the
+// raw 32 KiB of its cylinder once (TMA, 128-byte swizzle) and makes 4 tiles from it (residue pairs {0,4}, {2,6},
+// {1,5}, {3,7}), each a 128 x 64 x 512 GEMM per digit (16 tcgen05.mma of K = 32) into one of two TMEM accumulator
+// slots that rotate under the three digit passes.
 //
 // Warp roles (768 threads, 1 CTA / SM):
-//   warps 0-1     MMA issuers (one lane each: hi / lo digit)  warps 2-3    raw-block stagers (cp.async -> mbarrier)
+//   warps 0-1     MMA issuers (warp w owns accumulator slot w)   warps 2-3   raw-block staging (one lane, TMA)
 //   warps 4-7     operand preparation (integer butterflies -> K-major B tile), weight loads into TMEM
-//   warps 8-15    accumulator drain (tcgen05.ld), digit recombination, combine, twiddle, FFT-16, DSMEM send;
+//   warps 8-15    accumulator drain (tcgen05.ld), digit recombination, E +- O'/sqrt2, DSMEM send;
 //                 warps 8-11 take even tiles, 12-15 odd tiles; warp % 4 = TMEM lane quarter = destination CTA
-//   warps 16-23   receive side: E-W Horner, detect, accumulate; item epilogue (normalise, quantise, store)
-// All hand-overs are mbarriers (local, or remote through mapa for the two cluster-level ones).
+//   warps 16-23   receive side: E-W Horner, twiddle, FFT-16, detect, accumulate; frame end (normalise, quantise, store)
+// Hand-overs: mbarriers where an asynchronous unit or another CTA signals (TMA, tcgen05.commit, st.async, remote
+// arrive), named barriers for the two latency-critical local ones (slot drained, B tile written).
 #pragma once
 #include <cuda.h>            // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
@@ -453,8 +455,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
     if (warp < 2) {
         // ============================== MMA issuers: warp w owns accumulator slot w ==============================
         // Digit pass pi = 3 tau + p of tile tau goes to slot pi & 1 (two 64-column slots rotate under the three passes:
-        // weights 384 + accumulators 128 = all 512 columns).  D = s32, A = s8, B = s8, K-major, N = 64, M = 128.  Every
-        // pass ACCUMULATES onto what the last drain left in the slot (the magic constant, see drain_pass).
+        // weights 384 + accumulators 128 = all 512 columns).  D = s32, A = s8, B = s8, K-major, N = 64, M = 128.
         constexpr uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
         // Slot barriers are kept per drain group (g = tau & 1), so that every waiter sees the phases of its barrier in
         // order; the issuer waits for the drain of the slot's PREVIOUS use, whichever group that was.
