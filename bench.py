@@ -298,8 +298,7 @@ def run_cuda(args):
                      "peak_measured": peak_ffma2, "frac_of_measured": ach / peak_ffma2 if peak_ffma2 else None,
                      "peak_measured_note": f"chime_bf_measure_fp32_peak in this run: FFMA {peak_ffma:.1f}, FFMA2 "
                                            f"{peak_ffma2:.1f} TFLOP/s",
-                     "kernel": ("chime4::umma_beamform_kernel" if args.upchan == 128
-                                else "chime::beamform_fused_kernel"), "kernel_ms": kern_ms,
+                     "kernel": f"chime4::umma_beamform_kernel<{args.upchan}>", "kernel_ms": kern_ms,
                      "flops_per_chan_sample": fft_flops,
                      "note": f"FP32 peak = 148 SM x 128 lanes x 2 x {sm_mhz:.0f} MHz ({peak_kind} sm_max_mhz); "
                              "nominal FFT flops (5 n log2 n) per BASELINE north_star",

@@ -79,9 +79,8 @@ typedef struct {
     int exact_pointing;          /* 0: nearest bin of the zero-padded transform.
                                     1: exact chromatic alignment ("beam interpolation"): beam m is phased
                                     to its desired pointing itself, exp(-2 pi i n f d sin(theta_m) / c0); zero_pad then
-                                    only defines the index table that chime_bf_get_ns_index reports.  upchan_len 128
-                                    only (the tensor-core N-S transform takes any steering vector);
-                                    CHIME_BF_E_UNSUPPORTED (NULL plan) otherwise. */
+                                    only defines the index table that chime_bf_get_ns_index reports (the tensor-core
+                                    N-S transform takes any steering vector). */
 } chime_bf_params;
 
 chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *params);
@@ -181,7 +180,7 @@ int chime_bf_dedisperse_beams(void *cuda_stream, const uint8_t *beams_u8, int n_
  * UDP packet format"; the paper gives no formula -- reading F4 of DESIGN.md): a packet is the 32 consecutive N-S beams
  * x 16 fine channels (512 intensities) of one (channel, frame, E-W beam); its scale and offset follow from its own
  * data, scale = 16 / sigma (1 if sigma = 0), offset = 128 - mean * scale, u8 = sat(rne(I * scale + offset)), so that
- * I ~ (u8 - offset) / scale.  Statistics in fp32.  upchan_len 128 only (CHIME_BF_E_UNSUPPORTED otherwise).
+ * I ~ (u8 - offset) / scale.  Statistics in fp32.
  *   out_u8        DEVICE, as chime_bf_execute
  *   scale_offset  DEVICE, [C][n_frames][4][8][2] float (scale, offset) per packet, 8-byte aligned, caller-owned
  */

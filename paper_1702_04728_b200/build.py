@@ -6,7 +6,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libchime_bf.so")
 _SOURCES = ["chime_bf.cu"]
-_DEPS = ["chime_bf.cu", "beamform_kernel.cuh", "int_butterflies.cuh", "fp32_peak.cuh", "fft_regs.cuh", "dedisperse_kernel.cuh", "umma_beamform_kernel.cuh", os.path.join("..", "..", "include", "chime_bf.h")]
+_DEPS = ["chime_bf.cu", "beam_major.cuh", "int_butterflies.cuh", "fp32_peak.cuh", "fft_regs.cuh", "dedisperse_kernel.cuh", "umma_beamform_kernel.cuh", os.path.join("..", "..", "include", "chime_bf.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]

@@ -12,7 +12,7 @@
 #include <cstring>
 #include <vector>
 
-#include "beamform_kernel.cuh"
+#include "beam_major.cuh"
 #include "dedisperse_kernel.cuh"
 #include "fp32_peak.cuh"
 #include "umma_beamform_kernel.cuh"
@@ -46,11 +46,6 @@ struct chime_bf_plan {
     double fref = 600.0, d_feed = 0.3048, d_cyl = 22.0;
     bool exact_pointing = false;  // steer to the desired pointing itself instead of the nearest bin
     double *d_turns = nullptr;    // [C][256] phase step per feed (cycles) of the desired pointings, exact pointing only
-    float2 *d_wp = nullptr;
-    int16_t *d_slot = nullptr;
-    int16_t *d_slot_of_m = nullptr;
-    float2 *d_tw_np = nullptr;
-    float2 *d_tw_u = nullptr;
     // staging for execute_host
     uint8_t *d_stage_in = nullptr;
     uint8_t *d_stage_out = nullptr;
@@ -65,8 +60,7 @@ struct chime_bf_plan {
     int32_t *d_delay_stream = nullptr;
     int dd_D = -1, dd_L = 0;
     long long dd_t0 = 0;
-    // tensor-core N-S path (umma_beamform_kernel.cuh; upchan_len 128, any zero_pad)
-    bool use_umma = false;
+    // tensor-core N-S path (umma_beamform_kernel.cuh)
     uint32_t *d_wq = nullptr;     // TMEM images of the three-digit integer weights, 3 MiB per channel
     int4 *d_rowsum = nullptr;
     float2 *d_beta = nullptr;     // [C][4] E-W phase step of beam e
@@ -131,10 +125,10 @@ bool upload_on(T **dst, const std::vector<T> &src, cudaStream_t st) {
     return true;
 }
 
-// a4: index table J (eq. (1),(2)), compaction of the distinct selected bins into slots.
+// a4: index table J (eq. (1),(2)): the clamped bin of every beam; it decides the phase of the beam's weight row.
 bool build_index_tables(chime_bf_plan *pl, cudaStream_t st) {
+    (void)st;
     const int C = pl->C, NP = pl->NP, P = NP / 256;
-    std::vector<int16_t> slot((size_t)C * NP), slot_of_m((size_t)C * 256);
     pl->J.resize((size_t)C * 256);
     for (int c = 0; c < C; ++c) {
         const double f = pl->freq[c];
@@ -142,46 +136,8 @@ bool build_index_tables(chime_bf_plan *pl, cudaStream_t st) {
         for (int m = 0; m < 256; ++m)
             J[m] = !pl->ns_sin.empty() ? ns_bin_sintheta(NP, f, pl->d_feed, pl->ns_sin[m])
                                        : ns_bin(P, m, f, pl->fref, NP);
-        int16_t *sl = &slot[(size_t)c * NP];
-        std::fill(sl, sl + NP, (int16_t)-1);
-        for (int m = 0; m < 256; ++m) sl[J[m]] = 0;
-        int16_t ns = 0;
-        for (int j = 0; j < NP; ++j)
-            if (sl[j] == 0) sl[j] = ns++;
-        for (int m = 0; m < 256; ++m) slot_of_m[(size_t)c * 256 + m] = sl[J[m]];
     }
-    return upload_on(&pl->d_slot, slot, st) && upload_on(&pl->d_slot_of_m, slot_of_m, st);
-}
-
-// a2 + a5 folded weights (and their tensor-core fragments) from the plan's gains and E-W angles.
-bool build_weight_tables(chime_bf_plan *pl, cudaStream_t st) {
-    const int C = pl->C;
-    const double d_cyl = pl->d_cyl;
-    struct { const float *gains; const double *ew_angles_deg; } p = {pl->gains.empty() ? nullptr : pl->gains.data(), pl->ew_deg};
-    std::vector<float2> wp((size_t)C * 2 * 4 * 4 * 256);
-    for (int c = 0; c < C; ++c) {
-        const double f = pl->freq[c];
-        // a2+a5 folded: W'[pol][e][cyl][feed] = exp(-2 pi i f x_cyl sin(phi_e)/c0) * g[pol][cyl][feed]
-        for (int e = 0; e < 4; ++e) {
-            const double s = std::sin(p.ew_angles_deg[e] * kPi / 180.0);
-            for (int cy = 0; cy < 4; ++cy) {
-                const double ph = -2.0 * kPi * (f * 1e6) * ((double)cy * d_cyl) * s / kC0;
-                const double wr = std::cos(ph), wi = std::sin(ph);
-                for (int pol = 0; pol < 2; ++pol)
-                    for (int n = 0; n < 256; ++n) {
-                        double gr = 1.0, gi = 0.0;
-                        if (p.gains) {
-                            const float *g = p.gains + (((size_t)c * 2048) + (pol * 4 + cy) * 256 + n) * 2;
-                            gr = g[0];
-                            gi = g[1];
-                        }
-                        wp[((((size_t)c * 2 + pol) * 4 + e) * 4 + cy) * 256 + n] =
-                            make_float2((float)(wr * gr - wi * gi), (float)(wr * gi + wi * gr));
-                    }
-            }
-        }
-    }
-    return upload_on(&pl->d_wp, wp, st);
+    return true;
 }
 
 // Tensor-core path: the E-W phase steps (a5) -- 32 bytes per channel, all a re-pointing of the E-W beams uploads.
@@ -252,7 +208,7 @@ bool build_umma_weights(chime_bf_plan *pl, cudaStream_t st) {
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-bool encode_input_map(CUtensorMap *map, const uint8_t *in, size_t rows) {
+bool encode_input_map(CUtensorMap *map, const uint8_t *in, size_t rows, int box_rows) {
     static EncodeTiledFn fn = nullptr;
     if (fn == nullptr) {
         void *p = nullptr;
@@ -265,7 +221,7 @@ bool encode_input_map(CUtensorMap *map, const uint8_t *in, size_t rows) {
     }
     const cuuint64_t dims[2] = {2048, (cuuint64_t)rows};
     const cuuint64_t strides[1] = {2048};
-    const cuuint32_t box[2] = {128, 128};
+    const cuuint32_t box[2] = {128, (cuuint32_t)box_rows};   // one feed half of a block of upchan_len samples
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t *>(in), dims, strides, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -278,9 +234,9 @@ bool encode_input_map(CUtensorMap *map, const uint8_t *in, size_t rows) {
 }
 
 bool build_tables(chime_bf_plan *pl) {
-    const int NP = pl->NP, U = pl->U;
+    const int U = pl->U;
     if (!build_index_tables(pl, nullptr)) return false;
-    if (pl->use_umma) {
+    {
         std::vector<float2> tw128(128);
         for (int k = 0; k < 128; ++k) {
             const double a = -2.0 * kPi * (double)k / 128.0;
@@ -291,12 +247,25 @@ bool build_tables(chime_bf_plan *pl) {
         for (int rho = 0; rho < 8; ++rho)
             for (int u = 0; u < 16; ++u) twr[rho * 16 + u] = tw128[(rho * u) & 127];
         CUDA_TRY(cudaMemcpyToSymbol(chime4::c_twr, twr.data(), sizeof(float2) * 128));
-        CUDA_TRY(cudaFuncSetAttribute(chime4::umma_beamform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, chime4::kSmemBytes));
+        std::vector<float2> twr256(8 * 32), w32(16);
+        for (int rho = 0; rho < 8; ++rho)
+            for (int u = 0; u < 32; ++u) {
+                const double a = -2.0 * kPi * (double)(rho * u) / 256.0;
+                twr256[rho * 32 + u] = make_float2((float)std::cos(a), (float)std::sin(a));
+            }
+        for (int u = 0; u < 16; ++u) {
+            const double a = -2.0 * kPi * (double)u / 32.0;
+            w32[u] = make_float2((float)std::cos(a), (float)std::sin(a));
+        }
+        CUDA_TRY(cudaMemcpyToSymbol(chime4::c_twr256, twr256.data(), sizeof(float2) * 256));
+        CUDA_TRY(cudaMemcpyToSymbol(chime4::c_w32, w32.data(), sizeof(float2) * 16));
+        const void *kfn = U == 128 ? (const void *)chime4::umma_beamform_kernel<128> : (const void *)chime4::umma_beamform_kernel<256>;
+        CUDA_TRY(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, chime4::kSmemBytes));
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(4 * 148);
         cfg.blockDim = dim3(chime4::kThreads);
         cfg.dynamicSmemBytes = chime4::kSmemBytes;
-        CUDA_TRY(cudaOccupancyMaxActiveClusters(&pl->max_clusters, chime4::umma_beamform_kernel, &cfg));
+        CUDA_TRY(cudaOccupancyMaxActiveClusters(&pl->max_clusters, kfn, &cfg));
         if (pl->max_clusters < 1) { set_err("plan_create: no cluster of 4 CTAs fits on this device"); return false; }
         CUDA_TRY(cudaMalloc((void **)&pl->d_scratch, (size_t)pl->max_clusters * 4 * chime4::kMaxChunkFrames * 128 * 16 * sizeof(float)));
         CUDA_TRY(cudaHostAlloc((void **)&pl->h_status, 128 * sizeof(int), cudaHostAllocMapped));   // survives a trapped kernel
@@ -306,19 +275,6 @@ bool build_tables(chime_bf_plan *pl) {
         CUDA_TRY(cudaMalloc((void **)&pl->d_peer_out, 64 * sizeof(uint8_t *)));
         return build_ew_table(pl, nullptr) && build_umma_weights(pl, nullptr);
     }
-    if (!build_weight_tables(pl, nullptr)) return false;
-    std::vector<float2> tw_np(NP), tw_u(U);
-    for (int k = 0; k < NP; ++k) {
-        const double a = -2.0 * kPi * (double)k / (double)NP;
-        tw_np[k] = make_float2((float)std::cos(a), (float)std::sin(a));
-    }
-    for (int k = 0; k < U; ++k) {
-        const double a = -2.0 * kPi * (double)k / (double)U;
-        tw_u[k] = make_float2((float)std::cos(a), (float)std::sin(a));
-    }
-    CUDA_TRY(cudaMalloc((void **)&pl->d_delay, (size_t)pl->C * 16 * sizeof(int32_t)));
-    CUDA_TRY(cudaMalloc((void **)&pl->d_peer_out, 64 * sizeof(uint8_t *)));
-    return upload(&pl->d_tw_np, tw_np) && upload(&pl->d_tw_u, tw_u);
 }
 
 // Dispersion delay of fine channel (c, g) relative to f_ref, in output frames (reading F1):
@@ -343,20 +299,6 @@ int dedisp_table(const double *freq, int C, int U, double dm, double fref_mhz, s
     return mx;
 }
 
-template <int P, int RAD>
-bool prepare_kernel() {
-    CUDA_TRY(cudaFuncSetAttribute(chime::beamform_fused_kernel<P, RAD>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)chime::smem_bytes<P>()));
-    return true;
-}
-
-template <int P, int RAD>
-cudaError_t launch(const chime::KernelParams &kp, int n_cta, cudaStream_t st) {
-    chime::beamform_fused_kernel<P, RAD><<<n_cta, chime::kThreads, chime::smem_bytes<P>(), st>>>(kp);
-    return cudaGetLastError();
-}
-
 int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, float *out_f32, int chan0 = 0,
         int n_chan = -1, int frame0 = 0, int n_fr = -1, uint8_t *const *peer_out = nullptr, int n_peers = 0,
         int chan_global0 = 0, float *packet_so = nullptr) {
@@ -375,28 +317,8 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         set_err("execute: buffers must be 16-byte aligned");
         return CHIME_BF_E_ALIGNMENT;
     }
-    chime::KernelParams kp;
-    kp.in = reinterpret_cast<const uint32_t *>(in);
-    kp.out_u8 = out_u8;
-    kp.out_f32 = out_f32;
-    kp.wp = pl->d_wp;
-    kp.slot = pl->d_slot;
-    kp.slot_of_m = pl->d_slot_of_m;
-    kp.tw_np = pl->d_tw_np;
-    kp.tw_u = pl->d_tw_u;
-    kp.n_time = pl->T;
-    kp.n_frames = pl->R;
-    kp.chan0 = chan0;
-    kp.frame0 = frame0;
-    kp.n_frames_launch = n_fr;
-    kp.peer_out = peer_out;
-    kp.n_peers = n_peers;
-    kp.chan_global0 = chan_global0;
-    kp.norm = pl->norm;
-    kp.qscale = pl->norm * pl->scale;
-    kp.qoffset = pl->offset;
     cudaStream_t st = (cudaStream_t)stream;
-    if (pl->use_umma) {
+    {
         chime4::Params up;
         up.in = in;
         up.out_u8 = out_u8;
@@ -428,8 +350,9 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         const long long n_items = (long long)n_chan * ((n_fr + chunk - 1) / chunk) * 2;
         const int n_cl = (int)std::min<long long>(n_items, pl->max_clusters);
         CUtensorMap tmap;
-        if (!encode_input_map(&tmap, in, (size_t)pl->C * pl->T)) return CHIME_BF_E_CUDA;
-        chime4::umma_beamform_kernel<<<4 * n_cl, chime4::kThreads, chime4::kSmemBytes, st>>>(up, tmap);
+        if (!encode_input_map(&tmap, in, (size_t)pl->C * pl->T, pl->U)) return CHIME_BF_E_CUDA;
+        if (pl->U == 128) chime4::umma_beamform_kernel<128><<<4 * n_cl, chime4::kThreads, chime4::kSmemBytes, st>>>(up, tmap);
+        else chime4::umma_beamform_kernel<256><<<4 * n_cl, chime4::kThreads, chime4::kSmemBytes, st>>>(up, tmap);
         const cudaError_t e4 = cudaGetLastError();
         if (e4 != cudaSuccess) {
             set_err("kernel launch failed: %s", cudaGetErrorString(e4));
@@ -437,17 +360,6 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         }
         return CHIME_BF_OK;
     }
-    const int n_cta = n_chan * n_fr * 4;
-    cudaError_t e = cudaErrorInvalidValue;
-    const int P = pl->NP / 256, RAD = pl->U / 32;
-    if (P == 1 && RAD == 8) e = launch<1, 8>(kp, n_cta, st);
-    else if (P == 2 && RAD == 8) e = launch<2, 8>(kp, n_cta, st);
-    else if (P == 4 && RAD == 8) e = launch<4, 8>(kp, n_cta, st);
-    if (e != cudaSuccess) {
-        set_err("kernel launch failed: %s", cudaGetErrorString(e));
-        return CHIME_BF_E_CUDA;
-    }
-    return CHIME_BF_OK;
 }
 
 int launch_dedisperse(void *stream, const uint8_t *beams_u8, int C, int R, int n_beams, const std::vector<int32_t> &tab,
@@ -530,12 +442,6 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     pl->offset = p.scale > 0.f ? p.offset : 128.0f;
     pl->norm = (float)(1.0 / (256.0 * 4.0 * (double)p.upchan_len));
     pl->exact_pointing = p.exact_pointing != 0;
-    if (pl->exact_pointing && p.upchan_len != 128) {
-        set_err("plan_create: exact_pointing needs upchan_len 128");
-        delete pl;
-        return nullptr;
-    }
-    pl->use_umma = p.upchan_len == 128;   // upchan 256 runs the fp32 kernel of beamform_kernel.cuh
     cudaGetDevice(&pl->device);
     pl->fref = p.f_ref_mhz > 0 ? p.f_ref_mhz : 600.0;
     pl->d_feed = p.feed_spacing_m > 0 ? p.feed_spacing_m : 0.3048;
@@ -553,7 +459,6 @@ chime_bf_plan *chime_bf_plan_create_ex(const chime_bf_params *pp) {
     if (p.ns_sin_theta) pl->ns_sin.assign(p.ns_sin_theta, p.ns_sin_theta + 256);
     for (int e = 0; e < 4; ++e) pl->ew_deg[e] = p.ew_angles_deg[e];
     bool ok = build_tables(pl);
-    ok = ok && prepare_kernel<1, 8>() && prepare_kernel<2, 8>() && prepare_kernel<4, 8>();
     if (!ok) {
         chime_bf_destroy(pl);
         return nullptr;
@@ -581,7 +486,6 @@ int chime_bf_execute(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, ui
 int chime_bf_execute_packets(chime_bf_plan *plan, void *stream, const uint8_t *in_u8, uint8_t *out_u8,
                              float *scale_offset) {
     if (!plan || !scale_offset || !out_u8) { set_err("execute_packets: null argument"); return CHIME_BF_E_INVALID_ARG; }
-    if (!plan->use_umma) { set_err("execute_packets: upchan_len 128 only"); return CHIME_BF_E_UNSUPPORTED; }
     if ((uintptr_t)scale_offset & 7) { set_err("execute_packets: scale_offset must be 8-byte aligned"); return CHIME_BF_E_ALIGNMENT; }
     return run(plan, stream, in_u8, out_u8, nullptr, 0, -1, 0, -1, nullptr, 0, 0, scale_offset);
 }
@@ -685,15 +589,13 @@ int chime_bf_update_gains(chime_bf_plan *pl, void *stream, const float *gains) {
     if (gains && !gains_finite(gains, (size_t)pl->C * 2048 * 2)) { set_err("update_gains: gains must be finite"); return CHIME_BF_E_INVALID_ARG; }
     if (gains) pl->gains.assign(gains, gains + (size_t)pl->C * 2048 * 2);
     else pl->gains.clear();
-    if (pl->use_umma) return build_umma_weights(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
-    return build_weight_tables(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
+    return build_umma_weights(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
 }
 
 int chime_bf_update_ew_angles(chime_bf_plan *pl, void *stream, const double *ew_angles_deg) {
     if (!pl || !ew_angles_deg) { set_err("update_ew_angles: null argument"); return CHIME_BF_E_INVALID_ARG; }
     for (int e = 0; e < 4; ++e) pl->ew_deg[e] = ew_angles_deg[e];
-    if (pl->use_umma) return build_ew_table(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
-    return build_weight_tables(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
+    return build_ew_table(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
 }
 
 int chime_bf_update_pointings(chime_bf_plan *pl, void *stream, double f_ref_mhz, const double *ns_sin_theta) {
@@ -710,8 +612,7 @@ int chime_bf_update_pointings(chime_bf_plan *pl, void *stream, double f_ref_mhz,
         if (f_ref_mhz > 0) pl->fref = f_ref_mhz;
     }
     if (!build_index_tables(pl, (cudaStream_t)stream)) return CHIME_BF_E_CUDA;
-    if (pl->use_umma) return build_umma_weights(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
-    return CHIME_BF_OK;
+    return build_umma_weights(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
 }
 
 int chime_bf_dedisp_delays(const chime_bf_plan *pl, double dm, double f_ref_mhz, int32_t *host_out, int *n_out) {
@@ -916,11 +817,6 @@ int chime_bf_launches_per_execute(const chime_bf_plan *plan) { return plan ? 1 :
 
 void chime_bf_destroy(chime_bf_plan *pl) {
     if (!pl) return;
-    cudaFree(pl->d_wp);
-    cudaFree(pl->d_slot);
-    cudaFree(pl->d_slot_of_m);
-    cudaFree(pl->d_tw_np);
-    cudaFree(pl->d_tw_u);
     cudaFree(pl->d_stage_in);
     cudaFree(pl->d_stage_out);
     cudaFree(pl->d_delay);

@@ -7,6 +7,8 @@ namespace chime4 {
 
 __constant__ float2 c_tw128[128];  // exp(-2 pi i k / 128), uploaded at plan creation
 __constant__ float2 c_twr[8][16];  // [rho][u'] = exp(-2 pi i rho u' / 128): the same values in the order the time stage reads them
+__constant__ float2 c_twr256[8][32];  // upchan 256: [rho][u'] = exp(-2 pi i rho u' / 256)
+__constant__ float2 c_w32[16];        // upchan 256: exp(-2 pi i u / 32)
 
 // a1: byte = ((re + 8) << 4) | (im + 8): the offset-binary real and imaginary parts of four inputs
 // packed in one register, split by nibble masks into one value per byte.  This is THE decode of the hot path

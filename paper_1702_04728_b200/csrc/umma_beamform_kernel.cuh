@@ -43,7 +43,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "beamform_kernel.cuh"       // chime::beam_major_dst
+#include "beam_major.cuh"            // chime::beam_major_dst
 #include "int_butterflies.cuh"       // chime4::int_bfly4, c_twr
 #include "fft_regs.cuh"
 
@@ -199,19 +199,22 @@ __device__ __forceinline__ void bar_sync_named(int id, int n) { asm volatile("ba
 // K byte 32 j + i (i < 16): first half of feed 16 j + i, 32 j + 16 + i: second half; variant 0 = [re | im],
 // variant 1 = [im | -re]; signed bytes (the packed butterflies run on biased bytes, bias 64 (A, O') or 32 (E), which is
 // removed at the end).  Layout [kc = K/16][row group 8][8 rows][16 B].
-template <int TT>
-__device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned char *bop, const int pw, const int lane) {
+// U = 256: a block is 256 samples, t = u' + 32 k with u' = 16 h + (0 .. 15): the tile takes the 16 values of u' of half
+// h, the block sits in shared memory as [feed half][256 rows][128 B] (64 KiB, both raw buffers).
+template <int TT, int U>
+__device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned char *bop, const int pw, const int lane, const int h) {
     constexpr int R4 = (TT == 0) ? 0 : (TT == 1) ? 2 : (TT == 2) ? 1 : 3;
     constexpr uint32_t H40 = 0x40404040u, H80 = 0x80808080u;
     const int j = 4 * pw + (lane >> 3);                 // 16-feed chunk
     const int x7 = lane & 7;
-    const unsigned char *src = raw + (j >> 3) * 16384 + (((j & 7) ^ x7) << 4);
+    constexpr int kTap = U / 8;                         // row distance of the 8 taps of a residue
+    const unsigned char *src = raw + (j >> 3) * (U * 128) + (((j & 7) ^ x7) << 4) + (U == 256 ? h * 2048 : 0);
 #pragma unroll
     for (int it = 0; it < 2; ++it) {
         const int up = x7 + 8 * it;                     // u'
         uint4 q[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) q[k] = *reinterpret_cast<const uint4 *>(src + (up + 16 * k) * 128);
+        for (int k = 0; k < 8; ++k) q[k] = *reinterpret_cast<const uint4 *>(src + (up + kTap * k) * 128);
         uint32_t re0[4], im0[4], ng0[4], re1[4], im1[4], ng1[4];
 #pragma unroll
         for (int w = 0; w < 4; ++w) {
@@ -389,10 +392,44 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, con
         }
 }
 
+// Receive side, helpers of phase 2.  slot_free_arrive: "this warp has its part of receive slot s in registers" to the
+// four sending CTAs.  The arrive is made to depend on one word of every load (a[1], a[3], ... come from the 8 loads),
+// so that it cannot be issued while a load is still in flight.
+__device__ __forceinline__ void slot_free_arrive(const float2 (&a)[16], const uint32_t (&sf_remote)[4], const uint32_t s, const int lane) {
+    uint32_t dep;
+    asm volatile("{ .reg .b32 t0, t1;\n or.b32 t0, %1, %2;\n or.b32 t1, %3, %4;\n or.b32 t0, t0, t1;\n"
+                 " or.b32 t1, %5, %6;\n or.b32 t0, t0, t1;\n or.b32 t1, %7, %8;\n or.b32 t0, t0, t1;\n"
+                 " or.b32 %0, t0, 1; }"
+                 : "=r"(dep)
+                 : "r"(__float_as_uint(a[1].y)), "r"(__float_as_uint(a[3].y)), "r"(__float_as_uint(a[5].y)),
+                   "r"(__float_as_uint(a[7].y)), "r"(__float_as_uint(a[9].y)), "r"(__float_as_uint(a[11].y)),
+                   "r"(__float_as_uint(a[13].y)), "r"(__float_as_uint(a[15].y)));
+    dep = __reduce_or_sync(0xffffffffu, dep);   // every lane's loads
+    if (lane == 0 && dep != 0) {
+#pragma unroll
+        for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc] + 8 * s);
+    }
+}
+// FFT-16 over u' (input already twiddled), |.|^2 into the 16 fine channels: output bin q of the transform belongs to
+// fine channel (q + 8) & 15 for both up-channelisation lengths (U = 128: bin 8 q + rho of 128, 8 bins per fine channel;
+// U = 256: bins 8 (2 q) + rho and 8 (2 q + 1) + rho of 256, 16 per fine channel).
+__device__ __forceinline__ void fft16_detect(float2 (&a)[16], float (&acc)[16]) {
+    fft_dif<16>(a);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const int g = (bitrev(i, 4) + 8) & 15;
+        acc[g] = fmaf(a[i].x, a[i].x, fmaf(a[i].y, a[i].y, acc[g]));
+    }
+}
+
 // tmap: the packed baseband as a 2-D byte tensor [C * T rows][2048], box 128 bytes x 128 rows, 128-byte swizzle (the
 // layout prep_tile reads: 16-byte chunk index ^ (row & 7) inside every 128-byte row).
+// U = upchan_len (128 or 256): a frame is 3 blocks of U samples = 3 U / 32 tiles per polarisation.
+template <int U>
 __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(kThreads, 1)
 umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap) {
+    constexpr int kTilesPerFrame = 3 * U / 32;          // 12 or 24
+    constexpr int kRawBufs = U == 128 ? 2 : 1;          // raw blocks in flight (32 KiB each at U = 128, one of 64 KiB at U = 256)
     extern __shared__ __align__(1024) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     uint32_t rank;
@@ -466,7 +503,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
             for (int pol = 0; pol < 2; ++pol) {
                 PW(1, mbar_wait(BAR(B_W_READY), seg & 1, status, 1, seg);)
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const int ntiles = nf * 12;
+                const int ntiles = nf * kTilesPerFrame;
                 for (int t = 0; t < ntiles; ++t, ++tau) {
                     const uint32_t s = tau & 1, ph = (tau >> 1) & 1;
                     (void)ph;
@@ -521,25 +558,25 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         }
     } else if (warp < 4) {
         // ============================== raw-block stager: one lane, two TMA loads per block ==============================
-        // A block = 128 time samples x 256 bytes of (pol, cylinder): two boxes of 128 rows x 128 bytes (feeds 0-127,
-        // 128-255), each 16 KiB, swizzled by the copy engine.
+        // A block = U time samples x 256 bytes of (pol, cylinder): two boxes of U rows x 128 bytes (feeds 0-127, 128-255),
+        // swizzled by the copy engine (the tensor map's box is U rows high).
         if (warp == 2) {
             uint32_t beta = 0;
             ITEM_LOOP
                 for (int pol = 0; pol < 2; ++pol)
                     for (int fr = 0; fr < nf; ++fr)
                         for (int blk = 0; blk < 3; ++blk, ++beta) {
-                            const uint32_t b = beta & 1;
-                            PW(4, mbar_wait(BAR(B_RAW_EMPTY + b), ((beta >> 1) & 1) ^ 1, status, 4, beta);)
+                            const uint32_t b = beta % kRawBufs;
+                            PW(4, mbar_wait(BAR(B_RAW_EMPTY + b), ((beta / kRawBufs) & 1) ^ 1, status, 4, beta);)
                             if (elect_one()) {
-                                const int row = c * prm.n_time + ((fr0 + fr) * 3 + blk) * 128;
+                                const int row = c * prm.n_time + ((fr0 + fr) * 3 + blk) * U;
                                 const int col = pol * 1024 + (int)rank * 256;
                                 const uint32_t dst = smem_u32(smem + kOfsRaw) + b * kRawBytes, bar = BAR(B_RAW_FULL + b);
-                                mbar_expect_tx(bar, kRawBytes);
+                                mbar_expect_tx(bar, U * 256);
                                 asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                                              :: "r"(dst), "l"(&tmap), "r"(col), "r"(row), "r"(bar) : "memory");
                                 asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                                             :: "r"(dst + 16384), "l"(&tmap), "r"(col + 128), "r"(row), "r"(bar) : "memory");
+                                             :: "r"(dst + U * 128), "l"(&tmap), "r"(col + 128), "r"(row), "r"(bar) : "memory");
                             }
                             __syncwarp();
                         }
@@ -572,11 +609,12 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                 ++seg;
                 for (int fr = 0; fr < nf; ++fr)
                     for (int blk = 0; blk < 3; ++blk, ++beta) {
-                        const uint32_t b = beta & 1;
-                        PW(7, mbar_wait(BAR(B_RAW_FULL + b), (beta >> 1) & 1, status, 7, beta);)
+                        const uint32_t b = beta % kRawBufs;
+                        PW(7, mbar_wait(BAR(B_RAW_FULL + b), (beta / kRawBufs) & 1, status, 7, beta);)
                         const unsigned char *raw = smem + kOfsRaw + b * kRawBytes;
 #pragma unroll 1
-                        for (int tt = 0; tt < 4; ++tt, ++tau) {
+                        for (int th = 0; th < U / 32; ++th, ++tau) {   // U = 256: (residue pair tt, half h) with h fastest
+                            const int tt = U == 128 ? th : th >> 1, h = th & 1;
                             const uint32_t s = tau & 1;
                             PW(8, mbar_wait(BAR(B_BOP_EMPTY + s), ((tau >> 1) & 1) ^ 1, status, 8, tau);)
                             unsigned char *bop = smem + kOfsBop + s * kBopBytes;
@@ -584,10 +622,10 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                             if (prm.n_time < 0)
 #endif
                             switch (tt) {
-                                case 0: prep_tile<0>(raw, bop, pw, lane); break;
-                                case 1: prep_tile<1>(raw, bop, pw, lane); break;
-                                case 2: prep_tile<2>(raw, bop, pw, lane); break;
-                                default: prep_tile<3>(raw, bop, pw, lane); break;
+                                case 0: prep_tile<0, U>(raw, bop, pw, lane, h); break;
+                                case 1: prep_tile<1, U>(raw, bop, pw, lane, h); break;
+                                case 2: prep_tile<2, U>(raw, bop, pw, lane, h); break;
+                                default: prep_tile<3, U>(raw, bop, pw, lane, h); break;
                             }
                             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes -> tensor-core reads
                             asm volatile("bar.arrive %0, %1;" :: "r"(4 + s), "n"(kBopBarThreads) : "memory");   // named barrier: see slot_release
@@ -609,11 +647,11 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         uint32_t tau = 0;
         ITEM_LOOP
             for (int pol = 0; pol < 2; ++pol) {
-                const int ntiles = nf * 12;
+                const int ntiles = nf * kTilesPerFrame;
 #pragma unroll 1
                 for (int t = 0; t < ntiles; ++t, ++tau) {
                     if ((int)(tau & 1) != g) continue;
-                    epi_tile(t & 3, tlane, accf, n_use0, n_use1, tau, rslot, rfull, rank, lane, sfree, ((tau >> 1) & 1) ^ 1, status, prof_w);
+                    epi_tile(U == 128 ? (t & 3) : ((t >> 1) & 3), tlane, accf, n_use0, n_use1, tau, rslot, rfull, rank, lane, sfree, ((tau >> 1) & 1) ^ 1, status, prof_w);
                 }
             }
         }
@@ -647,7 +685,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll
                     for (int g = 0; g < 16; ++g) acc[g] = 0.f;
 #pragma unroll 1
-                    for (int t = 0; t < 12; ++t, ++tau) {
+                    for (int t = 0; t < kTilesPerFrame; ++t, ++tau) {
                         const uint32_t s = tau & 1;
                         PW(10, mbar_wait(BAR(B_RECV_FULL + s), (tau >> 1) & 1, status, 10, tau);)
                         if (rw == 0 && lane == 0) mbar_expect_tx(BAR(B_RECV_FULL + s), kRecvBytes);   // arm the slot's next tile
@@ -682,48 +720,69 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         }
-                        bar_sync_named(1, 256);
+                        if constexpr (U == 128) {
+                            bar_sync_named(1, 256);
 #if defined(CHIME_SKIP) && (CHIME_SKIP & 1)
-                        if (prm.n_time < 0)
+                            if (prm.n_time < 0)
 #endif
-                        {   // ---- phase 2: (beam, residue = res2, E-W beam = e2)
-                            const unsigned char *base = slot + ((e2 * 2 + res2) * 8) * 512;
+                            {   // ---- phase 2: (beam, residue = res2, E-W beam = e2)
+                                const unsigned char *base = slot + ((e2 * 2 + res2) * 8) * 512;
+                                float2 a[16];
+#pragma unroll
+                                for (int k = 0; k < 8; ++k) {
+                                    const float4 v = *reinterpret_cast<const float4 *>(base + k * 512);
+                                    a[2 * k] = make_float2(v.x, v.y);
+                                    a[2 * k + 1] = make_float2(v.z, v.w);
+                                }
+                                slot_free_arrive(a, sf_remote, s, lane);   // the slot is in registers: hand it back BEFORE the arithmetic
+                                // residue of (tile type, column set): {0,4}, {2,6}, {1,5}, {3,7}
+                                const int tt = t & 3;
+                                const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
+#pragma unroll
+                                for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr[rho][u]);
+                                fft16_detect(a, acc);
+                            }
+                        } else if (t & 1) {
+                            // U = 256: the FFT over u' has 32 points, u' = 16 h + u'': the tile of half 0 waits (E-W summed) in
+                            // the other slot, this one is half 1.  First stage across the halves, s = a0 + a1 and
+                            // d = (a0 - a1) W_32^{u''} (after the twiddles W_256^{rho u'}), then two FFT-16: s gives the
+                            // even bins, d the odd ones.  d waits in this thread's own cells of the slot meanwhile.
+                            bar_sync_named(1, 256);   // (covers phase 1 of the previous tile too: no barrier on even tiles)
+                            unsigned char *base1 = slot + ((e2 * 2 + res2) * 8) * 512;
+                            const unsigned char *base0 = base1 + (s ? -kRecvBytes : kRecvBytes);
+                            const int tt = (t >> 1) & 3;
+                            const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
                             float2 a[16];
 #pragma unroll
                             for (int k = 0; k < 8; ++k) {
-                                const float4 v = *reinterpret_cast<const float4 *>(base + k * 512);
+                                const float4 v0 = *reinterpret_cast<const float4 *>(base0 + k * 512);
+                                const float4 v1 = *reinterpret_cast<const float4 *>(base1 + k * 512);
+                                float2 d[2];
+#pragma unroll
+                                for (int j = 0; j < 2; ++j) {
+                                    const int u = 2 * k + j;
+                                    float2 p0 = j ? make_float2(v0.z, v0.w) : make_float2(v0.x, v0.y);
+                                    float2 p1 = j ? make_float2(v1.z, v1.w) : make_float2(v1.x, v1.y);
+                                    if (u > 0) p0 = chime::cmul(p0, c_twr256[rho][u]);
+                                    p1 = chime::cmul(p1, c_twr256[rho][16 + u]);
+                                    a[u] = chime::cadd(p0, p1);
+                                    d[j] = chime::csub(p0, p1);
+                                    if (u > 0) d[j] = chime::cmul(d[j], c_w32[u]);
+                                }
+                                const uint32_t oa = smem_u32(base1 + k * 512);
+                                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(oa), "f"(d[0].x), "f"(d[0].y) : "memory");
+                                asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" :: "r"(oa), "f"(d[1].x), "f"(d[1].y) : "memory");
+                            }
+                            slot_free_arrive(a, sf_remote, s ^ 1, lane);   // half 0's slot is consumed
+                            fft16_detect(a, acc);
+#pragma unroll
+                            for (int k = 0; k < 8; ++k) {
+                                const float4 v = *reinterpret_cast<const float4 *>(base1 + k * 512);
                                 a[2 * k] = make_float2(v.x, v.y);
                                 a[2 * k + 1] = make_float2(v.z, v.w);
                             }
-                            // The slot is in registers: hand it back to the four senders BEFORE the arithmetic.  The
-                            // arrive is made to depend on one word of every load, so that it cannot be issued while a
-                            // load is still in flight.
-                            {
-                                uint32_t dep;
-                                asm volatile("{ .reg .b32 t0, t1;\n or.b32 t0, %1, %2;\n or.b32 t1, %3, %4;\n or.b32 t0, t0, t1;\n"
-                                             " or.b32 t1, %5, %6;\n or.b32 t0, t0, t1;\n or.b32 t1, %7, %8;\n or.b32 t0, t0, t1;\n"
-                                             " or.b32 %0, t0, 1; }"
-                                             : "=r"(dep)
-                                             : "r"(__float_as_uint(a[1].y)), "r"(__float_as_uint(a[3].y)), "r"(__float_as_uint(a[5].y)),
-                                               "r"(__float_as_uint(a[7].y)), "r"(__float_as_uint(a[9].y)), "r"(__float_as_uint(a[11].y)),
-                                               "r"(__float_as_uint(a[13].y)), "r"(__float_as_uint(a[15].y)));
-                                dep = __reduce_or_sync(0xffffffffu, dep);   // every lane's loads
-                                if (lane == 0 && dep != 0) {
-#pragma unroll
-                                    for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc] + 8 * s);
-                                }
-                            }
-                            // residue of (tile type, column set): {0,4}, {2,6}, {1,5}, {3,7}
-                            const int tt = t & 3;
-                            const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
-#pragma unroll
-                            for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr[rho][u]);
-                            fft_dif<16>(a);
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) {
-                                const int g = (bitrev(i, 4) + 8) & 15;
-                                acc[g] = fmaf(a[i].x, a[i].x, fmaf(a[i].y, a[i].y, acc[g]));
-                            }
+                            slot_free_arrive(a, sf_remote, s, lane);
+                            fft16_detect(a, acc);
                         }
                     }
                     // ---- frame end: a9 sum of the two residue halves (+ pol 0), normalise, a10 quantise, 16-byte store per beam

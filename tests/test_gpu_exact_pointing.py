@@ -85,6 +85,23 @@ def test_exact_pointing_explicit_grid_and_repointing(bf, orc):
     plan.destroy()
 
 
-def test_exact_pointing_needs_upchan_128(bf):
-    with pytest.raises(bf.ChimeBfError, match="exact_pointing"):
-        bf.plan_create_ex(1, n_time=768, upchan_len=256, exact_pointing=True)
+def test_exact_pointing_upchan_256(bf, orc):
+    """The tensor-core N-S transform serves both up-channelisation lengths, so exact pointing does too."""
+    C, U = 2, 256
+    T = 2 * 3 * U
+    freqs = np.array([779.296875, 433.984375])
+    seed = synth.config_seed(4) + 19
+    gains = synth.gains(seed, C, flagged_frac=0.05)
+    b = synth.noise_bytes(seed, C, T)
+    plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, n_time=T, upchan_len=U, exact_pointing=True)
+    out_f32 = plan.execute_f32(b.cuda()).cpu().numpy()
+    out_u8 = plan.execute(b.cuda()).cpu().numpy()
+    hb = b.numpy()
+    worst = 0.0
+    for (c, R) in [(0, 1), (1, 0)]:
+        I = orc.cell_exact(hb[c, 3 * U * R:3 * U * (R + 1)], float(freqs[c]), gains=gains[c], U=U)
+        worst = max(worst, float((np.abs(out_f32[c, R] - I).max(axis=-1) / I.mean(axis=-1)).max()))
+        d = np.abs(out_u8[c, R].astype(int) - orc.quantize(I).astype(int))
+        assert d.max() <= 1 and (d != 0).mean() <= U8_FRAC
+    assert worst <= REL_TOL, worst
+    plan.destroy()

@@ -45,13 +45,27 @@ def test_packets_match_oracle(bf, orc, NP):
     plan.destroy()
 
 
-def test_packets_zero_input_and_unsupported(bf):
+def test_packets_zero_input(bf):
     plan = bf.plan_create_ex(1, n_time=384)
     z = torch.full((1, 384, 2048), 0x88, dtype=torch.uint8, device="cuda")
     u8, so = plan.execute_packets(z)
     assert torch.all(u8 == 128) and torch.all(so[..., 0] == 1.0) and torch.all(so[..., 1] == 128.0)
     plan.destroy()
-    plan = bf.plan_create_ex(1, n_time=768, upchan_len=256)
-    with pytest.raises(bf.ChimeBfError):
-        plan.execute_packets(torch.zeros((1, 768, 2048), dtype=torch.uint8, device="cuda"))
+
+
+def test_packets_upchan_256(bf, orc):
+    C, U = 1, 256
+    T = 2 * 3 * U
+    freqs = np.array([650.390625])
+    seed = synth.config_seed(4) + 23
+    gains = synth.gains(seed, C, flagged_frac=0.05)
+    b = synth.noise_bytes(seed, C, T)
+    plan = bf.plan_create_ex(C, freq_mhz=freqs, gains=gains, n_time=T, upchan_len=U)
+    u8, so = plan.execute_packets(b.cuda())
+    u8, so = u8.cpu().numpy(), so.cpu().numpy()
+    I, _ = orc.cell(b.numpy()[0, 3 * U:6 * U], float(freqs[0]), gains=gains[0], U=U)
+    q, so_ref = orc.packet_quantize(I)
+    assert np.allclose(so[0, 1], so_ref, rtol=2e-5, atol=1e-3)
+    d = np.abs(u8[0, 1].astype(int) - q.astype(int))
+    assert d.max() <= 1 and (d != 0).mean() <= 1e-3
     plan.destroy()
