@@ -1,8 +1,8 @@
 // Fourth-generation fused CHIME/FRB beamformer kernel for sm_100a: the N-S transform (a3 + a4, with the gains a2
 // folded in) runs on the 5th-generation tensor cores as an exact integer GEMM (tcgen05.mma kind::i8), the E-W sum (a5)
 // is an all-to-all over distributed shared memory inside a cluster of 4 CTAs, and the time transform (a7), detection,
-// integration and quantisation (a8-a10) run on the FP32 pipe around it.  upchan_len = 128, any zero_pad (the padding
-// factor only changes the weights).  PAPER.md:51-53 (the three kernels), :59-61 (N-S transform), :84-86 (up-channelise).
+// integration and quantisation (a8-a10) run on the FP32 pipe around it.  Any zero_pad (the padding factor only changes
+// the weights); upchan_len 128 is described below, 256 (template parameter U) where it differs (prep_tile, receive side).  PAPER.md:51-53 (the three kernels), :59-61 (N-S transform), :84-86 (up-channelise).
 //
 // Mathematics.  All operators before |.|^2 are linear and act on different axes, so they commute:
 //   1. time, first stage, on the raw 4-bit integers (exact, packed four feeds per register): with t = u' + 16 k,
