@@ -114,12 +114,14 @@ int chime_bf_execute_host(chime_bf_plan *plan, void *cuda_stream, const uint8_t 
  * precision exactly as plan creation does and copies them into the plan's existing device allocations,
  * ordered on `cuda_stream`: executes enqueued on that stream after the call see the new tables, executes
  * enqueued before it the old ones.  The caller must not have executes of this plan in flight on OTHER
- * streams.  No allocation, no plan rebuild.  Return CHIME_BF_OK or a negative code.
+ * streams.  No allocation, no plan rebuild.  The host-side copies (what chime_bf_get_ns_index reports) change
+ * with the call and are put back if it fails; the small tables are copied from pageable host memory, so the call may
+ * block the host until earlier work on `cuda_stream` has drained.  Return CHIME_BF_OK or a negative code.
  *   update_gains       gains: HOST [C][2048][2] float, copied; NULL = unit gains
  *   update_ew_angles   ew_angles_deg: HOST [4] double (tracking E-W beams: call once per pointing update)
  *   update_pointings   ns_sin_theta: HOST [256] double explicit pointings sin(theta_m) in [-1, 1], or NULL
  *                      to use the native 256-point grid at f_ref_mhz (<= 0 keeps the current f_ref).
- *                      Rebuilds the clamped index table J (eq. (1),(2)) and its slot maps.
+ *                      Rebuilds the clamped index table J (eq. (1),(2)) and the N-S weights on the device.
  */
 int chime_bf_update_gains(chime_bf_plan *plan, void *cuda_stream, const float *gains);
 int chime_bf_update_ew_angles(chime_bf_plan *plan, void *cuda_stream, const double *ew_angles_deg);

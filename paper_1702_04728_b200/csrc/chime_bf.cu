@@ -533,6 +533,12 @@ int chime_bf_execute_host(chime_bf_plan *pl, void *stream, const uint8_t *in_hos
     }
     if (e != cudaSuccess) {
         set_err("execute_host: %s", cudaGetErrorString(e));
+        // a half-finished first-call set-up must not be mistaken for a finished one by the next call
+        for (cudaEvent_t ev : pl->copy_done)
+            if (ev) cudaEventDestroy(ev);
+        pl->copy_done.clear();
+        if (pl->entry) { cudaEventDestroy(pl->entry); pl->entry = nullptr; }
+        if (pl->copy_stream) { cudaStreamDestroy(pl->copy_stream); pl->copy_stream = nullptr; }
         return CHIME_BF_E_CUDA;
     }
     // Pipeline by channel group (channels are independent; up to 8 groups): the copy stream uploads group k + 1
@@ -587,19 +593,31 @@ int chime_bf_execute_host(chime_bf_plan *pl, void *stream, const uint8_t *in_hos
 int chime_bf_update_gains(chime_bf_plan *pl, void *stream, const float *gains) {
     if (!pl) { set_err("update_gains: null plan"); return CHIME_BF_E_INVALID_ARG; }
     if (gains && !gains_finite(gains, (size_t)pl->C * 2048 * 2)) { set_err("update_gains: gains must be finite"); return CHIME_BF_E_INVALID_ARG; }
+    std::vector<float> old;
+    old.swap(pl->gains);   // the host copy follows the device tables: put back if the rebuild fails
     if (gains) pl->gains.assign(gains, gains + (size_t)pl->C * 2048 * 2);
-    else pl->gains.clear();
-    return build_umma_weights(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
+    if (build_umma_weights(pl, (cudaStream_t)stream)) return CHIME_BF_OK;
+    pl->gains.swap(old);
+    return CHIME_BF_E_CUDA;
 }
 
 int chime_bf_update_ew_angles(chime_bf_plan *pl, void *stream, const double *ew_angles_deg) {
     if (!pl || !ew_angles_deg) { set_err("update_ew_angles: null argument"); return CHIME_BF_E_INVALID_ARG; }
-    for (int e = 0; e < 4; ++e) pl->ew_deg[e] = ew_angles_deg[e];
-    return build_ew_table(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
+    double old[4];
+    for (int e = 0; e < 4; ++e) {
+        old[e] = pl->ew_deg[e];
+        pl->ew_deg[e] = ew_angles_deg[e];
+    }
+    if (build_ew_table(pl, (cudaStream_t)stream)) return CHIME_BF_OK;
+    for (int e = 0; e < 4; ++e) pl->ew_deg[e] = old[e];
+    return CHIME_BF_E_CUDA;
 }
 
 int chime_bf_update_pointings(chime_bf_plan *pl, void *stream, double f_ref_mhz, const double *ns_sin_theta) {
     if (!pl) { set_err("update_pointings: null plan"); return CHIME_BF_E_INVALID_ARG; }
+    const std::vector<double> old_sin = pl->ns_sin;
+    const std::vector<int32_t> old_J = pl->J;
+    const double old_fref = pl->fref;
     if (ns_sin_theta) {
         for (int m = 0; m < 256; ++m)
             if (!(ns_sin_theta[m] >= -1.0 && ns_sin_theta[m] <= 1.0)) {
@@ -611,8 +629,11 @@ int chime_bf_update_pointings(chime_bf_plan *pl, void *stream, double f_ref_mhz,
         pl->ns_sin.clear();
         if (f_ref_mhz > 0) pl->fref = f_ref_mhz;
     }
-    if (!build_index_tables(pl, (cudaStream_t)stream)) return CHIME_BF_E_CUDA;
-    return build_umma_weights(pl, (cudaStream_t)stream) ? CHIME_BF_OK : CHIME_BF_E_CUDA;
+    if (build_index_tables(pl, (cudaStream_t)stream) && build_umma_weights(pl, (cudaStream_t)stream)) return CHIME_BF_OK;
+    pl->ns_sin = old_sin;   // the index table chime_bf_get_ns_index reports stays the one the device weights were built from
+    pl->J = old_J;
+    pl->fref = old_fref;
+    return CHIME_BF_E_CUDA;
 }
 
 int chime_bf_dedisp_delays(const chime_bf_plan *pl, double dm, double f_ref_mhz, int32_t *host_out, int *n_out) {
