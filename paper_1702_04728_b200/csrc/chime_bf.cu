@@ -342,10 +342,23 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         up.status = pl->d_status;
         up.scratch = pl->d_scratch;
         up.packet_so = reinterpret_cast<float2 *>(packet_so);
-        // frames per work item: as many as possible (the weights are reloaded twice per item), while the launch still
-        // has at least 8 items per cluster to balance the persistent grid
-        int chunk = chime4::kMaxChunkFrames;
-        while (chunk > 1 && (long long)n_chan * ((n_fr + chunk - 1) / chunk) * 2 < 8LL * pl->max_clusters) chunk >>= 1;
+        // Frames per work item.  An item costs 2 x tiles_per_frame_and_pol x chunk tiles plus two weight reloads (~4 tile
+        // times each, measured), and the persistent grid runs ceil(items / clusters) rounds: take the chunk length that
+        // minimises rounds x item cost (long chunks amortise the reloads, short ones balance the grid).
+        int chunk = 1;
+        {
+            const long long tiles_pf = 2LL * 3 * (pl->U / 32);
+            long long best = -1;
+            for (int cf = chime4::kMaxChunkFrames; cf >= 1; cf >>= 1) {
+                const long long items = (long long)n_chan * ((n_fr + cf - 1) / cf) * 2;
+                const long long rounds = (items + pl->max_clusters - 1) / pl->max_clusters;
+                const long long cost = rounds * (tiles_pf * std::min(cf, n_fr) + 8);
+                if (best < 0 || cost < best) {
+                    best = cost;
+                    chunk = cf;
+                }
+            }
+        }
         up.chunk_frames = chunk;
         const long long n_items = (long long)n_chan * ((n_fr + chunk - 1) / chunk) * 2;
         const int n_cl = (int)std::min<long long>(n_items, pl->max_clusters);
