@@ -672,6 +672,8 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         float *ost = reinterpret_cast<float *>(smem + kOfsOut) + (e2 * 32 + lane) * 17;
         float4 *scr = reinterpret_cast<float4 *>(prm.scratch + ((size_t)blockIdx.x * kMaxChunkFrames * 128 + e2 * 32 + lane) * 16);
         uint32_t tau = 0;
+        uint64_t l2_keep;
+        asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(l2_keep));
         ITEM_LOOP
             float2 be[4];
 #pragma unroll
@@ -796,11 +798,15 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                         for (int g = 0; g < 16; ++g) acc[g] += ost[g];
                         if (pol == 0) {
 #pragma unroll
-                            for (int k = 0; k < 4; ++k) scr[fr * 128 * 4 + k] = make_float4(acc[4 * k], acc[4 * k + 1], acc[4 * k + 2], acc[4 * k + 3]);
+                            for (int k = 0; k < 4; ++k)   // parked in L2 (evict_last: 17 MB for the whole grid must survive up to 16 frames of input streaming past)
+                                asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;"
+                                             :: "l"(scr + fr * 128 * 4 + k), "f"(acc[4 * k]), "f"(acc[4 * k + 1]), "f"(acc[4 * k + 2]), "f"(acc[4 * k + 3]), "l"(l2_keep) : "memory");
                         } else {
 #pragma unroll
                             for (int k = 0; k < 4; ++k) {
-                                const float4 v = scr[fr * 128 * 4 + k];
+                                float4 v;
+                                asm volatile("ld.global.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;"
+                                             : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(scr + fr * 128 * 4 + k), "l"(l2_keep) : "memory");
                                 acc[4 * k] = (acc[4 * k] + v.x) * nrm;
                                 acc[4 * k + 1] = (acc[4 * k + 1] + v.y) * nrm;
                                 acc[4 * k + 2] = (acc[4 * k + 2] + v.z) * nrm;
