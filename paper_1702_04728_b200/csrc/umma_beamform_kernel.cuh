@@ -209,7 +209,7 @@ __device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned cha
     const int x7 = lane & 7;
     constexpr int kTap = U / 8;                         // row distance of the 8 taps of a residue
     const unsigned char *src = raw + (j >> 3) * (U * 128) + (((j & 7) ^ x7) << 4) + (U == 256 ? h * 2048 : 0);
-#pragma unroll
+#pragma unroll 1
     for (int it = 0; it < 2; ++it) {
         const int up = x7 + 8 * it;                     // u'
         uint4 q[8];
