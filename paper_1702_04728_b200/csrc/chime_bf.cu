@@ -62,7 +62,6 @@ struct chime_bf_plan {
     long long dd_t0 = 0;
     // tensor-core N-S path (umma_beamform_kernel.cuh)
     uint32_t *d_wq = nullptr;     // TMEM images of the three-digit integer weights, 3 MiB per channel
-    int4 *d_rowsum = nullptr;
     float2 *d_beta = nullptr;     // [C][4] E-W phase step of beam e
     float *d_inv_s2 = nullptr;    // [C]
     double *d_wscale = nullptr;   // [C] S_c
@@ -176,11 +175,9 @@ bool build_umma_weights(chime_bf_plan *pl, cudaStream_t st) {
     }
     if (!pl->d_wq) {
         CUDA_TRY(cudaMalloc((void **)&pl->d_wq, (size_t)C * 16 * chime4::kWqWordsPerSet * sizeof(uint32_t)));
-        CUDA_TRY(cudaMalloc((void **)&pl->d_rowsum, (size_t)C * 16 * 128 * sizeof(int4)));
     }
     chime4::WeightParams wp;
     wp.wq = pl->d_wq;
-    wp.rowsum = pl->d_rowsum;
     wp.gains = pl->gains.empty() ? nullptr : pl->d_gains;
     wp.J = pl->d_J;
     wp.turns = nullptr;
@@ -324,7 +321,6 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
         up.out_u8 = out_u8;
         up.out_f32 = out_f32;
         up.wq = pl->d_wq;
-        up.rowsum = pl->d_rowsum;
         up.beta = pl->d_beta;
         up.inv_s2 = pl->d_inv_s2;
         up.n_time = pl->T;
@@ -860,7 +856,6 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     cudaFree(pl->d_turns);
     cudaFree(pl->d_scratch);
     cudaFree(pl->d_wq);
-    cudaFree(pl->d_rowsum);
     cudaFree(pl->d_beta);
     cudaFree(pl->d_inv_s2);
     cudaFree(pl->d_wscale);

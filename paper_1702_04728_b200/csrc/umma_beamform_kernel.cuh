@@ -62,9 +62,8 @@ constexpr int kOfsOut = kOfsRecv + 2 * kRecvBytes;
 constexpr int kOutBytes = 4 * 32 * 17 * 4;      // [e][beam][16 + 1 pad] floats
 constexpr int kOfsBar = kOfsOut + kOutBytes;
 // mbarrier indices
-enum { B_RAW_FULL = 0, B_RAW_EMPTY = 2, B_BOP_FULL = 4, B_BOP_EMPTY = 6, B_TM_FULL = 8, B_TM_EMPTY = 10,
-       B_RECV_FULL = 12, B_SLOT_FREE = 14 /* [dest 4][slot 2] */, B_W_FREE = 22, B_W_READY = 23,
-       B_ACC_FULL = 24 /* [group 2][slot 2] */, B_ACC_EMPTY = 28, B_COUNT = 32 };
+enum { B_RAW_FULL = 0, B_RAW_EMPTY = 2, B_BOP_EMPTY = 6, B_RECV_FULL = 12, B_SLOT_FREE = 14 /* [dest 4][slot 2] */,
+       B_W_FREE = 22, B_W_READY = 23, B_ACC_FULL = 24 /* [group 2][slot 2] */, B_COUNT = 32 };
 constexpr int kSmemBytes = kOfsBar + B_COUNT * 8 + 16;
 
 constexpr int kDigits = 3;                      // signed 8-bit digits per weight (24-bit weights)
@@ -76,7 +75,6 @@ struct Params {
     uint8_t *out_u8;          // [C][R][4][256][16]
     float *out_f32;           // same layout, or nullptr
     const uint32_t *wq;       // [C][pol 2][cyl 4][tile 2][quarter 4][c32 12][i 32][lane 32]: TMEM images of the weights
-    const int4 *rowsum;       // [C][pol][cyl][tile][128] sum of the digits of each row (digit 2, 1, 0, unused)
     const float2 *beta;       // [C][4] E-W phase step per cylinder of beam e
     const float *inv_s2;      // [C] 1 / S_c^2 (weight scale)
     int n_time, n_frames;
@@ -133,17 +131,6 @@ __device__ __forceinline__ void mbar_timeout(int *status, int code, uint32_t inf
     __threadfence_system();
     for (long long t1 = clock64(); clock64() - t1 < 1500000000ll;) {}
     __trap();
-}
-// Latency-critical waits: test_wait does not park the warp, so the phase flip is seen within one poll.
-__device__ __forceinline__ void mbar_spin(uint32_t a, uint32_t parity, int *status, int code, uint32_t info = 0) {
-    uint32_t n = 0;
-    while (true) {
-        uint32_t ok;
-        asm volatile("{ .reg .pred p; mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
-        if (ok) break;
-        if (++n > (1u << 26)) mbar_timeout(status, code, info);
-    }
 }
 __device__ __forceinline__ void mbar_wait(uint32_t a, uint32_t parity, int *status, int code, uint32_t info = 0) {
     uint32_t n = 0;
@@ -344,11 +331,7 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, con
     for (int p = 0; p < 3; ++p) {
         const uint32_t slot = (tau + p) & 1;     // = (3 tau + p) & 1
         const uint32_t use = slot ? n_use1 : n_use0;
-#ifdef CHIME_SPINFULL
-        PW(9, mbar_spin(bar_full0 + 8 * slot, use & 1, status, 9, tau);)
-#else
         PW(9, mbar_wait(bar_full0 + 8 * slot, use & 1, status, 9, tau);)
-#endif
         n_use0 += 1 - slot;
         n_use1 += slot;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -443,7 +426,6 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         for (int s = 0; s < 2; ++s) {
             mbar_init(BAR(B_RAW_FULL + s), 1);    // one expect_tx arrive; the TMA reports the bytes
             mbar_init(BAR(B_RAW_EMPTY + s), 4);
-            mbar_init(BAR(B_BOP_FULL + s), 4);
             mbar_init(BAR(B_BOP_EMPTY + s), 2);
             mbar_init(BAR(B_RECV_FULL + s), 1);
         }
@@ -885,7 +867,6 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 constexpr int kWMax = 127 * 65536 + 127 * 256 + 127;   // largest 24-bit weight whose three digits fit in [-128, 127]
 struct WeightParams {
     uint32_t *wq;
-    int4 *rowsum;
     const float2 *gains;      // [C][2048] or nullptr (unit)
     const int32_t *J;         // [C][256]
     const double *turns;      // [C][256] exact pointing (turns per feed), or nullptr
@@ -901,7 +882,6 @@ __global__ void __launch_bounds__(128) build_weights_kernel(const WeightParams w
     const int J = wp.J[(size_t)c * 256 + m];
     const double x = wp.turns ? wp.turns[(size_t)c * 256 + m] : 0.0;
     uint32_t *dst = wp.wq + (size_t)set * kWqWordsPerSet + quarter * (kWCols * 32) + lane;
-    int sum[3] = {0, 0, 0};
     for (int n4 = 0; n4 < 64; ++n4) {
         uint32_t w1[3] = {0, 0, 0}, w2[3] = {0, 0, 0};   // digit 2 (top), 1, 0 of the first / second K half
         for (int b = 0; b < 4; ++b) {
@@ -930,9 +910,6 @@ __global__ void __launch_bounds__(128) build_weights_kernel(const WeightParams w
                 v = (v - d0) >> 8;
                 const int d1 = ((v + 128) & 255) - 128;
                 const int d2 = (v - d1) >> 8;
-                sum[0] += d2;
-                sum[1] += d1;
-                sum[2] += d0;
                 uint32_t *w = h ? w2 : w1;
                 w[0] |= (uint32_t)(d2 & 255) << (8 * b);
                 w[1] |= (uint32_t)(d1 & 255) << (8 * b);
@@ -948,7 +925,6 @@ __global__ void __launch_bounds__(128) build_weights_kernel(const WeightParams w
             put(128 * p + kw2, w2[p]);
         }
     }
-    wp.rowsum[(size_t)set * 128 + row] = make_int4(sum[0], sum[1], sum[2], 0);
 }
 
 }  // namespace chime4
