@@ -132,10 +132,11 @@ __device__ __forceinline__ void mbar_timeout(int *status, int code, uint32_t inf
     for (long long t1 = clock64(); clock64() - t1 < 1500000000ll;) {}
     __trap();
 }
-__device__ __forceinline__ void mbar_wait(uint32_t a, uint32_t parity, int *status, int code, uint32_t info = 0) {
+// (prm.status is read from the parameter bank on the cold path only: no register holds it while the warp works)
+__device__ __forceinline__ void mbar_wait(uint32_t a, uint32_t parity, const Params &prm, int code, uint32_t info = 0) {
     uint32_t n = 0;
     while (!mbar_try(a, parity))
-        if (++n > (1u << 20)) mbar_timeout(status, code, info);
+        if (++n > (1u << 20)) mbar_timeout(prm.status, code, info);
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
@@ -289,29 +290,34 @@ __device__ __forceinline__ void slot_release(const uint32_t slot, const int lane
     asm volatile("bar.arrive %0, %1;" :: "r"(2 + slot), "n"(kSlotBarThreads) : "memory");
 }
 
-template <int P>
+// W = columns per load: 32 (two round trips per pass; 64 + 32 registers at the drain's 112) or 16 (four round trips).
+// ptxas may still issue several loads before the arithmetic of the first and spill partial sums for it: W = 16 made
+// that worse, not better (measured on the U = 256 instantiation), so both run W = 32.
+template <int P, int W>
 __device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64], const uint32_t slot, const int lane, long long *t_rel = nullptr) {
     constexpr float kS = P == 1 ? 1.0f / 256.0f : 1.0f / 65536.0f;
 #pragma unroll
-    for (int hf = 0; hf < 2; ++hf) {   // hf = part: 32 columns at a time
-        uint32_t h[32];
-        tmem_ld32(tslot + 32 * hf, h);
+    for (int c = 0; c < 64 / W; ++c) {   // columns W c .. W c + W - 1: part = column / 32, j = column % 32
+        uint32_t h[W];
+        if constexpr (W == 32) tmem_ld32(tslot + W * c, h);
+        else tmem_ld16(tslot + W * c, h);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        if (hf == 1) {
+        if (c == 64 / W - 1) {
             slot_release(slot, lane);
 #ifdef CHIME_PROF
             *t_rel = clock64();
 #endif
         }
 #if defined(CHIME_SKIP) && (CHIME_SKIP & 4)
-        y[hf] = __uint_as_float(h[0] ^ h[31]);
+        y[c] = __uint_as_float(h[0] ^ h[W - 1]);
         if (lane > 32)
 #endif
 #pragma unroll
-        for (int j = 0; j < 32; ++j) {
-            const float f = __uint_as_float(h[j] + kMagicBits);   // (cvt.rn.f32.s32 instead: 5 % slower, measured)
-            if constexpr (P == 0) y[2 * j + hf] = f - kMagicSum;
-            else y[2 * j + hf] = fmaf(f, kS, y[2 * j + hf]);
+        for (int i = 0; i < W; ++i) {
+            const int col = W * c + i, part = col >> 5, j = col & 31;
+            const float f = __uint_as_float(h[i] + kMagicBits);   // (cvt.rn.f32.s32 instead: 5 % slower, measured)
+            if constexpr (P == 0) y[2 * j + part] = f - kMagicSum;
+            else y[2 * j + part] = fmaf(f, kS, y[2 * j + part]);
         }
     }
 }
@@ -322,18 +328,20 @@ __device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64],
 // folded into y and the slot handed back at once.  Odd-residue tiles (tt >= 2) combine E and O' here; the rest of the
 // time transform (twiddle, FFT-16) is linear and runs AFTER the E-W sum on the receiving side.
 // Receive slot layout: [cyl 4][res 2][u' pair 8][beam 32] x {re, im, re, im}.
-__device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, const uint32_t bar_full0,
-                                         uint32_t &n_use0, uint32_t &n_use1, const uint32_t tau, const uint32_t rslot, const uint32_t rbar,
-                                         const int cyl, const int lane, const uint32_t slot_free_bar,
-                                         const uint32_t sf_parity, int *status, long long *prof_w) {
+// Group g takes the tiles tau = 2 k + g: its passes use slots g, g ^ 1, g, so tile k is uses 2 k, 2 k + 1 of barrier
+// ACC_FULL[g][g] and use k of ACC_FULL[g][g ^ 1]: the parities are 0, k & 1, 1 -- no counters.  Everything that is only
+// needed after the three passes (destination addresses) is computed there: the drain runs at the edge of its registers.
+template <int W>
+__device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const uint32_t bar0, const uint32_t recv0, const uint32_t g,
+                                         const uint32_t q, const uint32_t tau, const int cyl, const int lane, const Params &prm,
+                                         long long *prof_w) {
     float y[64];
+    const uint32_t tlane = tb + ((32u * q) << 16), bar_full0 = bar0 + 8u * (B_ACC_FULL + 2 * g);
 #pragma unroll
     for (int p = 0; p < 3; ++p) {
-        const uint32_t slot = (tau + p) & 1;     // = (3 tau + p) & 1
-        const uint32_t use = slot ? n_use1 : n_use0;
-        PW(9, mbar_wait(bar_full0 + 8 * slot, use & 1, status, 9, tau);)
-        n_use0 += 1 - slot;
-        n_use1 += slot;
+        const uint32_t slot = p == 1 ? (g ^ 1) : g;     // = (3 tau + p) & 1
+        const uint32_t parity = p == 0 ? 0u : p == 1 ? ((tau >> 1) & 1) : 1u;
+        PW(9, mbar_wait(bar_full0 + 8 * slot, parity, prm, 9, tau);)
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t tslot = tlane + kWCols + 64 * slot;
 #ifdef CHIME_PROF
@@ -341,15 +349,15 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, con
 #endif
 #ifdef CHIME_PROF
         long long _t1 = 0;
-        if (p == 0) drain_pass<0>(tslot, y, slot, lane, &_t1);
-        else if (p == 1) drain_pass<1>(tslot, y, slot, lane, &_t1);
-        else drain_pass<2>(tslot, y, slot, lane, &_t1);
+        if (p == 0) drain_pass<0, W>(tslot, y, slot, lane, &_t1);
+        else if (p == 1) drain_pass<1, W>(tslot, y, slot, lane, &_t1);
+        else drain_pass<2, W>(tslot, y, slot, lane, &_t1);
         prof_w[6] += _t1 - _t0;
         prof_w[7] += clock64() - _t1;
 #else
-        if (p == 0) drain_pass<0>(tslot, y, slot, lane);
-        else if (p == 1) drain_pass<1>(tslot, y, slot, lane);
-        else drain_pass<2>(tslot, y, slot, lane);
+        if (p == 0) drain_pass<0, W>(tslot, y, slot, lane);
+        else if (p == 1) drain_pass<1, W>(tslot, y, slot, lane);
+        else drain_pass<2, W>(tslot, y, slot, lane);
 #endif
     }
     if (tt >= 2) {   // A_rho = E + O'/sqrt2 (set 0), A_{rho+4} = E - O'/sqrt2 (set 1)
@@ -361,7 +369,8 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, con
             y[32 + k] = fmaf(-s, o, e);
         }
     }
-    PW(5, mbar_wait(slot_free_bar, sf_parity, status, 5);)     // the destination has consumed this slot's previous tile
+    const uint32_t rslot = mapa(recv0 + g * kRecvBytes, q), rbar = mapa(bar0 + 8u * (B_RECV_FULL + g), q);
+    PW(5, mbar_wait(bar0 + 8u * (B_SLOT_FREE + 2 * q + g), ((tau >> 1) & 1) ^ 1, prm, 5);)     // the destination has consumed this slot's previous tile
     // Asynchronous stores: each reports its 16 bytes to the destination's mbarrier (complete_tx), so the receiver's
     // wait on that barrier is the only synchronisation: no fence, no arrive on the sending side.
 #pragma unroll
@@ -378,7 +387,9 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tlane, con
 // Receive side, helpers of phase 2.  slot_free_arrive: "this warp has its part of receive slot s in registers" to the
 // four sending CTAs.  The arrive is made to depend on one word of every load (a[1], a[3], ... come from the 8 loads),
 // so that it cannot be issued while a load is still in flight.
-__device__ __forceinline__ void slot_free_arrive(const float2 (&a)[16], const uint32_t (&sf_remote)[4], const uint32_t s, const int lane) {
+// sf_local = this CTA's own SLOT_FREE barrier of (its beams, slot s): the same offset in each source CTA (mapa at the
+// point of use: four live registers less on a role that runs at the edge of its 72).
+__device__ __forceinline__ void slot_free_arrive(const float2 (&a)[16], const uint32_t sf_local, const int lane) {
     uint32_t dep;
     asm volatile("{ .reg .b32 t0, t1;\n or.b32 t0, %1, %2;\n or.b32 t1, %3, %4;\n or.b32 t0, t0, t1;\n"
                  " or.b32 t1, %5, %6;\n or.b32 t0, t0, t1;\n or.b32 t1, %7, %8;\n or.b32 t0, t0, t1;\n"
@@ -390,7 +401,7 @@ __device__ __forceinline__ void slot_free_arrive(const float2 (&a)[16], const ui
     dep = __reduce_or_sync(0xffffffffu, dep);   // every lane's loads
     if (lane == 0 && dep != 0) {
 #pragma unroll
-        for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(sf_remote[sc] + 8 * s);
+        for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(mapa(sf_local, sc));
     }
 }
 // FFT-16 over u' (input already twiddled), |.|^2 into the 16 fine channels: output bin q of the transform belongs to
@@ -452,7 +463,6 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 
     const int n_chunks = (prm.n_frames_launch + prm.chunk_frames - 1) / prm.chunk_frames;
     const int n_items = prm.n_chan * n_chunks * 2;
-    int *const status = prm.status;
     long long prof_w[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
     const long long prof_t0 = clock64();
     (void)prof_t0;
@@ -483,7 +493,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         uint32_t n_mine = 0;               // passes issued to my slot
         ITEM_LOOP
             for (int pol = 0; pol < 2; ++pol) {
-                PW(1, mbar_wait(BAR(B_W_READY), seg & 1, status, 1, seg);)
+                PW(1, mbar_wait(BAR(B_W_READY), seg & 1, prm, 1, seg);)
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const int ntiles = nf * kTilesPerFrame;
                 for (int t = 0; t < ntiles; ++t, ++tau) {
@@ -549,7 +559,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                     for (int fr = 0; fr < nf; ++fr)
                         for (int blk = 0; blk < 3; ++blk, ++beta) {
                             const uint32_t b = beta % kRawBufs;
-                            PW(4, mbar_wait(BAR(B_RAW_EMPTY + b), ((beta / kRawBufs) & 1) ^ 1, status, 4, beta);)
+                            PW(4, mbar_wait(BAR(B_RAW_EMPTY + b), ((beta / kRawBufs) & 1) ^ 1, prm, 4, beta);)
                             if (elect_one()) {
                                 const int row = c * prm.n_time + ((fr0 + fr) * 3 + blk) * U;
                                 const int col = pol * 1024 + (int)rank * 256;
@@ -571,7 +581,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         ITEM_LOOP
             for (int pol = 0; pol < 2; ++pol) {
                 if (seg > 0) {
-                    PW(6, mbar_wait(BAR(B_W_FREE), (seg - 1) & 1, status, 6);)   // every MMA that read the old weights is done
+                    PW(6, mbar_wait(BAR(B_W_FREE), (seg - 1) & 1, prm, 6);)   // every MMA that read the old weights is done
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 }
                 {
@@ -592,13 +602,13 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                 for (int fr = 0; fr < nf; ++fr)
                     for (int blk = 0; blk < 3; ++blk, ++beta) {
                         const uint32_t b = beta % kRawBufs;
-                        PW(7, mbar_wait(BAR(B_RAW_FULL + b), (beta / kRawBufs) & 1, status, 7, beta);)
+                        PW(7, mbar_wait(BAR(B_RAW_FULL + b), (beta / kRawBufs) & 1, prm, 7, beta);)
                         const unsigned char *raw = smem + kOfsRaw + b * kRawBytes;
 #pragma unroll 1
                         for (int th = 0; th < U / 32; ++th, ++tau) {   // U = 256: (residue pair tt, half h) with h fastest
                             const int tt = U == 128 ? th : th >> 1, h = th & 1;
                             const uint32_t s = tau & 1;
-                            PW(8, mbar_wait(BAR(B_BOP_EMPTY + s), ((tau >> 1) & 1) ^ 1, status, 8, tau);)
+                            PW(8, mbar_wait(BAR(B_BOP_EMPTY + s), ((tau >> 1) & 1) ^ 1, prm, 8, tau);)
                             unsigned char *bop = smem + kOfsBop + s * kBopBytes;
 #if defined(CHIME_SKIP) && (CHIME_SKIP & 2)
                             if (prm.n_time < 0)
@@ -619,21 +629,16 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         }
     } else if (warp < 16) {
         // ============================== accumulator drain, FFT-16, DSMEM send ==============================
-        const int g = (warp - 8) >> 2, q = warp & 3;
-        const uint32_t tlane = tb + ((uint32_t)(32 * q) << 16);
-        const uint32_t rslot = mapa(smem_u32(smem + kOfsRecv) + g * kRecvBytes, q);
-        const uint32_t rfull = mapa(BAR(B_RECV_FULL + g), q);
-        const uint32_t sfree = BAR(B_SLOT_FREE + 2 * q + g);
-        const uint32_t accf = BAR(B_ACC_FULL + 2 * g);
-        uint32_t n_use0 = 0, n_use1 = 0;
+        const uint32_t g = (warp - 8) >> 2, q = warp & 3;
+        const uint32_t recv0 = smem_u32(smem + kOfsRecv);
         uint32_t tau = 0;
         ITEM_LOOP
             for (int pol = 0; pol < 2; ++pol) {
                 const int ntiles = nf * kTilesPerFrame;
 #pragma unroll 1
-                for (int t = 0; t < ntiles; ++t, ++tau) {
-                    if ((int)(tau & 1) != g) continue;
-                    epi_tile(U == 128 ? (t & 3) : ((t >> 1) & 3), tlane, accf, n_use0, n_use1, tau, rslot, rfull, rank, lane, sfree, ((tau >> 1) & 1) ^ 1, status, prof_w);
+                for (int t = ntiles; t > 0; --t, ++tau) {   // (tiles per frame and polarisation: a multiple of 8, so tau gives the tile type)
+                    if ((tau & 1) != g) continue;
+                    epi_tile<32>(U == 128 ? (tau & 3) : ((tau >> 1) & 3), tb, bar0, recv0, g, q, tau, rank, lane, prm, prof_w);
                 }
             }
         }
@@ -648,19 +653,12 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         // of (E-W beam, beam), park the polarisation-0 sums in a per-CTA scratch (L2) and finish the frame after pol 1.
         const int rw = warp - 16;
         const int res2 = rw & 1, e2 = rw >> 1;
-        uint32_t sf_remote[4];   // slot 0's barrier of this CTA's beams in each source CTA; slot 1's is 8 bytes further
-#pragma unroll
-        for (int s = 0; s < 4; ++s) sf_remote[s] = mapa(BAR(B_SLOT_FREE + 2 * rank), s);
-        float *ost = reinterpret_cast<float *>(smem + kOfsOut) + (e2 * 32 + lane) * 17;
-        float4 *scr = reinterpret_cast<float4 *>(prm.scratch + ((size_t)blockIdx.x * kMaxChunkFrames * 128 + e2 * 32 + lane) * 16);
+        const uint32_t sf0 = BAR(B_SLOT_FREE + 2 * rank);   // slot 0's barrier of this CTA's beams (in every source CTA); slot 1's is 8 bytes further
         uint32_t tau = 0;
-        uint64_t l2_keep;
-        asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(l2_keep));
         ITEM_LOOP
             float2 be[4];
 #pragma unroll
             for (int e = 0; e < 4; ++e) be[e] = __ldg(prm.beta + (size_t)c * 4 + e);
-            const float nrm = prm.norm * __ldg(prm.inv_s2 + c);
 #pragma unroll 1
             for (int pol = 0; pol < 2; ++pol) {
 #pragma unroll 1
@@ -671,7 +669,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll 1
                     for (int t = 0; t < kTilesPerFrame; ++t, ++tau) {
                         const uint32_t s = tau & 1;
-                        PW(10, mbar_wait(BAR(B_RECV_FULL + s), (tau >> 1) & 1, status, 10, tau);)
+                        PW(10, mbar_wait(BAR(B_RECV_FULL + s), (tau >> 1) & 1, prm, 10, tau);)
                         if (rw == 0 && lane == 0) mbar_expect_tx(BAR(B_RECV_FULL + s), kRecvBytes);   // arm the slot's next tile
                         unsigned char *slot = smem + kOfsRecv + s * kRecvBytes + lane * 16;
 #if defined(CHIME_SKIP) && (CHIME_SKIP & 1)
@@ -718,7 +716,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                                     a[2 * k] = make_float2(v.x, v.y);
                                     a[2 * k + 1] = make_float2(v.z, v.w);
                                 }
-                                slot_free_arrive(a, sf_remote, s, lane);   // the slot is in registers: hand it back BEFORE the arithmetic
+                                slot_free_arrive(a, sf0 + 8 * s, lane);   // the slot is in registers: hand it back BEFORE the arithmetic
                                 // residue of (tile type, column set): {0,4}, {2,6}, {1,5}, {3,7}
                                 const int tt = t & 3;
                                 const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
@@ -733,15 +731,14 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                             // even bins, d the odd ones.  d waits in this thread's own cells of the slot meanwhile.
                             bar_sync_named(1, 256);   // (covers phase 1 of the previous tile too: no barrier on even tiles)
                             unsigned char *base1 = slot + ((e2 * 2 + res2) * 8) * 512;
-                            const unsigned char *base0 = base1 + (s ? -kRecvBytes : kRecvBytes);
+                            unsigned char *base0 = base1 + (s ? -kRecvBytes : kRecvBytes);
                             const int tt = (t >> 1) & 3;
                             const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
-                            float2 a[16];
 #pragma unroll
                             for (int k = 0; k < 8; ++k) {
                                 const float4 v0 = *reinterpret_cast<const float4 *>(base0 + k * 512);
                                 const float4 v1 = *reinterpret_cast<const float4 *>(base1 + k * 512);
-                                float2 d[2];
+                                float2 sm[2], d[2];
 #pragma unroll
                                 for (int j = 0; j < 2; ++j) {
                                     const int u = 2 * k + j;
@@ -749,15 +746,26 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                                     float2 p1 = j ? make_float2(v1.z, v1.w) : make_float2(v1.x, v1.y);
                                     if (u > 0) p0 = chime::cmul(p0, c_twr256[rho][u]);
                                     p1 = chime::cmul(p1, c_twr256[rho][16 + u]);
-                                    a[u] = chime::cadd(p0, p1);
+                                    sm[j] = chime::cadd(p0, p1);
                                     d[j] = chime::csub(p0, p1);
                                     if (u > 0) d[j] = chime::cmul(d[j], c_w32[u]);
                                 }
-                                const uint32_t oa = smem_u32(base1 + k * 512);
-                                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(oa), "f"(d[0].x), "f"(d[0].y) : "memory");
-                                asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" :: "r"(oa), "f"(d[1].x), "f"(d[1].y) : "memory");
+                                // both branches wait in the thread's own cells (s in this slot, d in the other one), so that
+                                // the loop holds two points at a time and the FFTs run on the registers of U = 128
+                                const uint32_t o1 = smem_u32(base1 + k * 512), o0 = smem_u32(base0 + k * 512);
+                                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(o1), "f"(sm[0].x), "f"(sm[0].y) : "memory");
+                                asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" :: "r"(o1), "f"(sm[1].x), "f"(sm[1].y) : "memory");
+                                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(o0), "f"(d[0].x), "f"(d[0].y) : "memory");
+                                asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" :: "r"(o0), "f"(d[1].x), "f"(d[1].y) : "memory");
                             }
-                            slot_free_arrive(a, sf_remote, s ^ 1, lane);   // half 0's slot is consumed
+                            float2 a[16];
+#pragma unroll
+                            for (int k = 0; k < 8; ++k) {
+                                const float4 v = *reinterpret_cast<const float4 *>(base0 + k * 512);
+                                a[2 * k] = make_float2(v.x, v.y);
+                                a[2 * k + 1] = make_float2(v.z, v.w);
+                            }
+                            slot_free_arrive(a, sf0 + 8 * (s ^ 1), lane);   // half 0's slot is consumed
                             fft16_detect(a, acc);
 #pragma unroll
                             for (int k = 0; k < 8; ++k) {
@@ -765,10 +773,17 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                                 a[2 * k] = make_float2(v.x, v.y);
                                 a[2 * k + 1] = make_float2(v.z, v.w);
                             }
-                            slot_free_arrive(a, sf_remote, s, lane);
+                            slot_free_arrive(a, sf0 + 8 * s, lane);
                             fft16_detect(a, acc);
                         }
                     }
+                    // (pointers and the cache policy of the frame end are made here, once per frame: nothing of them is alive
+                    // while the tiles are processed, where this role runs at the edge of its registers)
+                    float *ost = reinterpret_cast<float *>(smem + kOfsOut) + (e2 * 32 + lane) * 17;
+                    float4 *scr = reinterpret_cast<float4 *>(prm.scratch + ((size_t)blockIdx.x * kMaxChunkFrames * 128 + e2 * 32 + lane) * 16);
+                    uint64_t l2_keep;
+                    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(l2_keep));
+                    const float nrm = prm.norm * __ldg(prm.inv_s2 + c);
                     // ---- frame end: a9 sum of the two residue halves (+ pol 0), normalise, a10 quantise, 16-byte store per beam
                     if (res2 == 0) {
 #pragma unroll
