@@ -178,6 +178,25 @@ int chime_bf_dedisperse_beams(void *cuda_stream, const uint8_t *beams_u8, int n_
                               int32_t *delay_scratch, uint32_t *out_u32, int n_out);
 
 /*
+ * chime_bf_dedisperse_beams for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same kernel and formula (reading F1), but the
+ * kernel's scratch -- the delay table [n_coarse][16] int32 -- lives in a file-scope device array of the library
+ * instead of a caller-owned buffer.  Limit: n_coarse <= CHIME_BF_NOALLOC_MAX_COARSE (1024 = the full band; the array is
+ * 64 KiB and every GPU that loads the library holds it until exit); a larger n_coarse is CHIME_BF_E_INVALID_ARG with a
+ * message.  The call allocates nothing on the device and frees nothing (no cudaMalloc / cudaFree / allocating library
+ * routine; on the host one thread-local table is sized on a thread's first call).  Arguments as
+ * chime_bf_dedisperse_beams without delay_scratch: beams_u8, out_u32 DEVICE and caller-owned; freq_mhz HOST.
+ * Every call on a device shares the one array and finds the previous call's table in it: each call rewrites the
+ * n_coarse*16 entries it uses on `cuda_stream` before its kernel reads them (and clears out_u32 when the channel loop
+ * is split), so calls that follow each other on one stream are safe; calls that OVERLAP on the GPU (different streams
+ * without an event between them) race on the table.
+ */
+#define CHIME_BF_NOALLOC_MAX_COARSE 1024
+int chime_bf_dedisperse_beams_noalloc(void *cuda_stream, const uint8_t *beams_u8, int n_coarse, const double *freq_mhz,
+                                      int n_frames, int n_beams, int upchan_len, double dm, double f_ref_mhz,
+                                      uint32_t *out_u32, int n_out);
+
+/*
  * chime_bf_execute with the packetiser's per-packet rescale ("rescaled to 8-bit integers ... in a custom
  * UDP packet format"; the paper gives no formula -- reading F4 of DESIGN.md): a packet is the 32 consecutive N-S beams
  * x 16 fine channels (512 intensities) of one (channel, frame, E-W beam); its scale and offset follow from its own

@@ -22,6 +22,7 @@ EXPORTS = [
     "chime_bf_dedisp_delays", "chime_bf_dedisperse", "chime_bf_execute_beam_major", "chime_bf_dedisperse_beams",
     "chime_bf_dedisp_delays_ex", "chime_bf_kernel_status", "chime_bf_measure_fp32_peak",
     "chime_bf_execute_packets", "chime_bf_dedisperse_stream_begin", "chime_bf_dedisperse_stream_push",
+    "chime_bf_dedisperse_beams_noalloc",
 ]
 
 
@@ -93,6 +94,8 @@ def load_library():
     lib.chime_bf_dedisp_delays_ex.argtypes = [vp, ci, ci, ctypes.c_double, ctypes.c_double, vp, ctypes.POINTER(ci)]
     lib.chime_bf_dedisperse_beams.restype = ci
     lib.chime_bf_dedisperse_beams.argtypes = [vp, vp, ci, vp, ci, ci, ci, ctypes.c_double, ctypes.c_double, vp, vp, ci]
+    lib.chime_bf_dedisperse_beams_noalloc.restype = ci
+    lib.chime_bf_dedisperse_beams_noalloc.argtypes = [vp, vp, ci, vp, ci, ci, ci, ctypes.c_double, ctypes.c_double, vp, ci]
     lib.chime_bf_kernel_status.restype = ci
     lib.chime_bf_kernel_status.argtypes = [vp]
     lib.chime_bf_measure_fp32_peak.restype = ci
@@ -328,6 +331,29 @@ def dedisperse_beams(beams_u8, freq_mhz, dm, upchan_len=128, f_ref_mhz=0.0, stre
     rc = load_library().chime_bf_dedisperse_beams(_stream_ptr(stream), beams_u8.data_ptr(), C, f.ctypes.data, R, nb,
                                                   upchan_len, float(dm), float(f_ref_mhz), scratch.data_ptr(),
                                                   out.data_ptr(), n_out)
+    if rc != 0:
+        raise ChimeBfError(f"chime_bf error {rc}: {last_error()}")
+    return out
+
+
+NOALLOC_MAX_COARSE = 1024
+
+
+def dedisperse_beams_noalloc(beams_u8, freq_mhz, dm, out, upchan_len=128, f_ref_mhz=0.0, stream=None):
+    """chime_bf_dedisperse_beams_noalloc: as dedisperse_beams, but nothing is allocated on the device -- the delay table
+    lives in the library's built-in device array (at most NOALLOC_MAX_COARSE channels) and the CALLER passes `out`,
+    int32 [n_beams][n_out] with n_out = R - max delay (dedisp_delays_ex).  Calls that overlap on the GPU race."""
+    import torch
+    assert beams_u8.is_cuda and beams_u8.dtype == torch.uint8 and beams_u8.is_contiguous() and beams_u8.dim() == 4
+    C, R, nb, nf = beams_u8.shape
+    assert nf == N_FINE
+    assert out.is_cuda and out.dtype == torch.int32 and out.is_contiguous() and out.dim() == 2 and out.shape[0] == nb
+    f = np.ascontiguousarray(freq_mhz, dtype=np.float64)
+    if f.size != C:
+        raise ValueError("freq_mhz must have one entry per coarse channel")
+    rc = load_library().chime_bf_dedisperse_beams_noalloc(_stream_ptr(stream), beams_u8.data_ptr(), C, f.ctypes.data, R,
+                                                          nb, upchan_len, float(dm), float(f_ref_mhz), out.data_ptr(),
+                                                          int(out.shape[1]))
     if rc != 0:
         raise ChimeBfError(f"chime_bf error {rc}: {last_error()}")
     return out

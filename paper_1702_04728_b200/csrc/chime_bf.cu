@@ -371,6 +371,33 @@ int run(chime_bf_plan *pl, void *stream, const uint8_t *in, uint8_t *out_u8, flo
     }
 }
 
+// Scratch of chime_bf_dedisperse_beams_noalloc: the delay table of the dedispersion kernel in a file-scope device array,
+// so that the call needs no allocation.  64 KiB per GPU that loads the library, until exit.  In host code the name is a
+// host-side stand-in, NOT a device address: noalloc_delay_table() asks the runtime for the address on the current
+// device (once per device) and the kernel gets that pointer.
+static __device__ __align__(256) int32_t g_noalloc_delay[CHIME_BF_NOALLOC_MAX_COARSE * 16];
+
+int32_t *noalloc_delay_table() {
+    constexpr int kMaxDev = 64;
+    static int32_t *ptr[kMaxDev] = {};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= kMaxDev) {
+        set_err("dedisperse_beams_noalloc: cudaGetDevice: %s (device %d)", cudaGetErrorString(e), dev);
+        return nullptr;
+    }
+    if (ptr[dev] == nullptr) {   // set-up, once per device, with that device current
+        int32_t *p = nullptr;
+        e = cudaGetSymbolAddress((void **)&p, g_noalloc_delay);
+        if (e != cudaSuccess || p == nullptr) {
+            set_err("dedisperse_beams_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+            return nullptr;
+        }
+        ptr[dev] = p;
+    }
+    return ptr[dev];
+}
+
 int launch_dedisperse(void *stream, const uint8_t *beams_u8, int C, int R, int n_beams, const std::vector<int32_t> &tab,
                       int32_t *d_delay, uint32_t *out_u32, int n_out) {
     cudaStream_t st = (cudaStream_t)stream;
@@ -763,6 +790,39 @@ int chime_bf_dedisperse_beams(void *stream, const uint8_t *beams_u8, int n_coars
         return CHIME_BF_E_INVALID_ARG;
     }
     return launch_dedisperse(stream, beams_u8, n_coarse, n_frames, n_beams, tab, delay_scratch, out_u32, n_out);
+}
+
+int chime_bf_dedisperse_beams_noalloc(void *stream, const uint8_t *beams_u8, int n_coarse, const double *freq_mhz,
+                                      int n_frames, int n_beams, int upchan_len, double dm, double f_ref_mhz,
+                                      uint32_t *out_u32, int n_out) {
+    if (!beams_u8 || !freq_mhz || !out_u32 || n_coarse < 1 || n_frames < 1 || !(dm >= 0)) {
+        set_err("dedisperse_beams_noalloc: bad argument");
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    if (n_coarse > CHIME_BF_NOALLOC_MAX_COARSE) {
+        set_err("dedisperse_beams_noalloc: n_coarse %d exceeds the built-in scratch (CHIME_BF_NOALLOC_MAX_COARSE = %d); "
+                "use chime_bf_dedisperse_beams with a caller-owned table", n_coarse, CHIME_BF_NOALLOC_MAX_COARSE);
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    if (n_beams < 32 || n_beams % 32 || (upchan_len != 128 && upchan_len != 256)) {
+        set_err("dedisperse_beams_noalloc: n_beams must be a positive multiple of 32, upchan_len 128 or 256");
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    if ((uintptr_t)beams_u8 & 15) { set_err("dedisperse_beams_noalloc: input must be 16-byte aligned"); return CHIME_BF_E_ALIGNMENT; }
+    static thread_local std::vector<int32_t> tab;   // host side: sized on the thread's first call, re-used afterwards
+    tab.reserve((size_t)CHIME_BF_NOALLOC_MAX_COARSE * 16);
+    const int mx = dedisp_table(freq_mhz, n_coarse, upchan_len, dm, f_ref_mhz, tab);
+    for (int32_t d : tab)
+        if (d < 0) { set_err("dedisperse_beams_noalloc: f_ref below a fine channel (negative delay)"); return CHIME_BF_E_INVALID_ARG; }
+    if (n_frames - mx < 1 || n_out != n_frames - mx) {
+        set_err("dedisperse_beams_noalloc: n_out must be n_frames - max delay = %d (got %d)", n_frames - mx, n_out);
+        return CHIME_BF_E_INVALID_ARG;
+    }
+    int32_t *d_delay = noalloc_delay_table();   // the device address of the array on the current device
+    if (d_delay == nullptr) return CHIME_BF_E_CUDA;
+    // launch_dedisperse rewrites tab.size() entries of the table on `stream` before the kernel reads them, and clears
+    // out_u32 when the channel loop is split: nothing of the previous call's contents is read.
+    return launch_dedisperse(stream, beams_u8, n_coarse, n_frames, n_beams, tab, d_delay, out_u32, n_out);
 }
 
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out) {
