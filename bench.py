@@ -311,6 +311,8 @@ def run_cuda(args):
         "gpu_launches": args.steps * plan.launches_per_execute,
         "clocks": clocks,
     }
+    if world == 1 and args.workload == "group":     # outside the timed region of the step: the (f1) kernel's own roofline
+        line["dedisp"] = dedisp_subrecords()
     if not args.no_cpu_baseline and world == 1:     # the oracle is timed on rank 0 at N = 1 only
         dt, cs, cores = oracle_sample(256)
         v = cs * BYTES_PER_CHAN_SAMPLE / dt / 1e9
@@ -382,6 +384,49 @@ def run_cfg3(args):
     print(json.dumps(line))
     st.destroy()
     return 0
+
+
+def dedisp_subrecords(steps=20):
+    """Sub-records of the default line: the dedispersion kernel on a configs[2]-shaped beam
+    array, uint8 [64 channels][1017 frames][1024 beams][16 fine] = 1.07 GB (>> L2), at DM 10 and DM 40, through
+    chime_bf_dedisperse_beams_noalloc (no allocation inside the timed region).  HBM-bound: achieved = algorithmic bytes
+    (input bytes on some track + uint32 output) / CUDA-event time per launch, against the measured HBM peak."""
+    import torch
+
+    import paper_1702_04728_b200 as bf
+    import synth
+
+    cfg = synth.CONFIGS[2]
+    C, R = cfg["n_coarse"], cfg["n_time"] // 384
+    freqs = synth.config_freqs(2)
+    g = torch.Generator(device="cuda").manual_seed(synth.config_seed(2))
+    beams = torch.randint(0, 256, (C, R, 1024, 16), dtype=torch.uint8, device="cuda", generator=g)
+    peaks, peak_kind = measured_peaks()
+    stream = torch.cuda.current_stream()
+    recs = []
+    for dm in (10.0, 40.0):
+        _, mx = bf.dedisp_delays_ex(freqs, dm)
+        n_out = R - mx
+        out = torch.empty((1024, n_out), dtype=torch.int32, device="cuda")
+        for _ in range(3):
+            bf.dedisperse_beams_noalloc(beams, freqs, dm, out, stream=stream)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            bf.dedisperse_beams_noalloc(beams, freqs, dm, out, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        nbytes = C * n_out * 1024 * 16 + out.numel() * 4
+        ach = nbytes / (ms * 1e-3) / 1e9
+        recs.append({"dm": dm, "n_out": n_out, "kernel": "chime_dd::dedisperse_kernel", "kernel_ms": ms, "steps": steps,
+                     "bound": "hbm", "achieved": ach, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
+                     "frac": ach / float(peaks["hbm_gbs"]), "algorithmic_bytes": nbytes, "peak_kind": peak_kind})
+        del out
+    del beams
+    torch.cuda.empty_cache()
+    return recs
 
 
 def run_dedisp(args):

@@ -305,6 +305,18 @@ class Plan:
             pass
 
 
+def dedisp_delays_ex(freq_mhz, dm, upchan_len=128, f_ref_mhz=0.0):
+    """chime_bf_dedisp_delays_ex -> (delay table int32 [C][16], max delay in output frames)."""
+    f = np.ascontiguousarray(freq_mhz, dtype=np.float64)
+    tab = np.zeros((f.size, N_FINE), dtype=np.int32)
+    mx = ctypes.c_int(0)
+    rc = load_library().chime_bf_dedisp_delays_ex(f.ctypes.data, int(f.size), upchan_len, float(dm), float(f_ref_mhz),
+                                                  tab.ctypes.data, ctypes.byref(mx))
+    if rc != 0:
+        raise ChimeBfError(f"chime_bf error {rc}: {last_error()}")
+    return tab, mx.value
+
+
 def dedisperse_beams(beams_u8, freq_mhz, dm, upchan_len=128, f_ref_mhz=0.0, stream=None):
     """chime_bf_dedisperse_beams: uint8 beams [C][R][n_beams][16] (any beam subset) -> int32 [n_beams][n_out].
     n_out = R - max delay comes from chime_bf_dedisp_delays_ex."""

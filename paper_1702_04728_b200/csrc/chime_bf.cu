@@ -419,7 +419,8 @@ int launch_dedisperse(void *stream, const uint8_t *beams_u8, int C, int R, int n
         if (n_split > 1) e = cudaMemsetAsync(out_u32, 0, (size_t)n_beams * n_out * sizeof(uint32_t), st);
         if (e == cudaSuccess) {
             dim3 grid(bt, tt, n_split);
-            chime_dd::dedisperse_kernel<<<grid, chime_dd::kThreads, 0, st>>>(dp);
+            if (n_beams == 1024) chime_dd::dedisperse_kernel<1024><<<grid, chime_dd::kThreads, 0, st>>>(dp);
+            else chime_dd::dedisperse_kernel<0><<<grid, chime_dd::kThreads, 0, st>>>(dp);
             e = cudaGetLastError();
         }
     }
@@ -745,7 +746,7 @@ int chime_bf_dedisperse_stream_push(chime_bf_plan *pl, void *stream, const uint8
     sp.c_per_split = (pl->C + n_split - 1) / n_split;
     n_split = (pl->C + sp.c_per_split - 1) / sp.c_per_split;
     cudaStream_t st = (cudaStream_t)stream;
-    chime_dd::dedisperse_stream_kernel<<<dim3(bt, tt, n_split), chime_dd::kThreads, 0, st>>>(sp);
+    chime_dd::dedisperse_stream_kernel<1024><<<dim3(bt, tt, n_split), chime_dd::kThreads, 0, st>>>(sp);
     chime_dd::dedisperse_emit_kernel<<<dim3((pl->R + 255) / 256, 1024), 256, 0, st>>>(sp);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_err("dedisperse_stream_push: %s", cudaGetErrorString(e)); return CHIME_BF_E_CUDA; }
