@@ -412,8 +412,27 @@ int launch_dedisperse(void *stream, const uint8_t *beams_u8, int C, int R, int n
         dp.n_out = n_out;
         dp.n_beams = n_beams;
         const int bt = n_beams / chime_dd::kBeamsPerCta, tt = (n_out + chime_dd::kTR - 1) / chime_dd::kTR;
-        // fill 148 SMs x 16 resident CTAs: split the channel loop when beams x time tiles are too few
-        int n_split = std::min(C, std::max(1, (148 * 16 + bt * tt - 1) / (bt * tt)));
+        // Split of the channel loop over blockIdx.z: the kernel is short (40 - 160 us), so what matters is that the grid
+        // is a whole number of waves of the resident CTAs (5 per SM at 90 registers).  Cost of a split = waves x
+        // (channels per CTA + ~4.5 channels' worth of fixed work per CTA: start-up latency, the final shuffles and
+        // atomics; fitted to a sweep of the split at DM 5 / 10 / 20 / 40 on the bench workload).
+        int n_split = 1;
+        {
+            const long long slots = 148LL * 5;
+            double best = -1.0;
+            for (int ns = 1; ns <= std::min(C, 16); ++ns) {
+                const int cps = (C + ns - 1) / ns, ns_eff = (C + cps - 1) / cps;
+                const long long waves = ((long long)bt * tt * ns_eff + slots - 1) / slots;
+                const double cost = (double)waves * ((double)cps + 4.5);
+                if (best < 0 || cost < best) {
+                    best = cost;
+                    n_split = ns_eff;
+                }
+            }
+        }
+#ifdef CHIME_DD_SWEEP
+        if (getenv("DD_SPLIT")) n_split = atoi(getenv("DD_SPLIT"));
+#endif
         dp.c_per_split = (C + n_split - 1) / n_split;
         n_split = (C + dp.c_per_split - 1) / dp.c_per_split;
         if (n_split > 1) e = cudaMemsetAsync(out_u32, 0, (size_t)n_beams * n_out * sizeof(uint32_t), st);

@@ -45,9 +45,11 @@ __global__ void __launch_bounds__(kThreads, 4) dedisperse_kernel(const Params p)
     const int n_valid = min(kTR, p.n_out - r0);      // ragged last tile
     const size_t frame_words = NB ? (size_t)NB * 4 : (size_t)p.n_beams * 4;
     const int c_lo = blockIdx.z * p.c_per_split, c_hi = min(p.C, c_lo + p.c_per_split);
+    int4 dl_next = *reinterpret_cast<const int4 *>(p.delay + c_lo * 16 + 4 * q);
 #pragma unroll 1
     for (int c = c_lo; c < c_hi; ++c) {
-        const int4 dl = *reinterpret_cast<const int4 *>(p.delay + c * 16 + 4 * q);
+        const int4 dl = dl_next;   // the next channel's delays are fetched under this channel's loads (one dependent latency less per channel)
+        if (c + 1 < c_hi) dl_next = *reinterpret_cast<const int4 *>(p.delay + (c + 1) * 16 + 4 * q);
         const uint32_t *base = p.in + (size_t)c * p.R * frame_words + (size_t)b * 4 + q;
         // One pass per delay value v of the quad: the lane adds the bytes whose delay is v with dp4a against a
         // 0/1 byte mask -- every word is loaded once per distinct delay of its quad (once, for most quads),
