@@ -411,35 +411,45 @@ int launch_dedisperse(void *stream, const uint8_t *beams_u8, int C, int R, int n
         dp.R = R;
         dp.n_out = n_out;
         dp.n_beams = n_beams;
-        const int bt = n_beams / chime_dd::kBeamsPerCta, tt = (n_out + chime_dd::kTR - 1) / chime_dd::kTR;
-        // Split of the channel loop over blockIdx.z: the kernel is short (40 - 160 us), so what matters is that the grid
-        // is a whole number of waves of the resident CTAs (5 per SM at 90 registers).  Cost of a split = waves x
-        // (channels per CTA + ~4.5 channels' worth of fixed work per CTA: start-up latency, the final shuffles and
-        // atomics; fitted to a sweep of the split at DM 5 / 10 / 20 / 40 on the bench workload).
-        int n_split = 1;
+        // Tile length and split of the channel loop over blockIdx.z.  The kernel is short (40 - 160 us), so what matters is
+        // that the grid is a whole number of waves of the resident CTAs (5 per SM with 32-sample tiles, 8 with 16-sample
+        // ones).  Cost of a choice = waves x (work of a CTA + its fixed work: start-up latency, the final shuffles and
+        // atomics -- ~4.5 channels' worth of a 32-sample tile, fitted to a sweep of the split at DM 5 / 10 / 20 / 40 on
+        // the bench workload), in units of one channel of a 32-sample tile per resident CTA slot.
+        const int bt = n_beams / chime_dd::kBeamsPerCta;
+        int tr = chime_dd::kTR, n_split = 1;
         {
-            const long long slots = 148LL * 5;
             double best = -1.0;
-            for (int ns = 1; ns <= std::min(C, 16); ++ns) {
-                const int cps = (C + ns - 1) / ns, ns_eff = (C + cps - 1) / cps;
-                const long long waves = ((long long)bt * tt * ns_eff + slots - 1) / slots;
-                const double cost = (double)waves * ((double)cps + 4.5);
-                if (best < 0 || cost < best) {
-                    best = cost;
-                    n_split = ns_eff;
+            for (int t = 32; t >= 16; t >>= 1) {
+                const long long slots = 148LL * (t == 32 ? 5 : 8);
+                const int tt_ = (n_out + t - 1) / t;
+                const double unit = (t == 32 ? 1.0 : 0.5 * 8.0 / 5.0);   // half the bytes per channel, but 8 CTAs share an SM instead of 5
+                for (int ns = 1; ns <= std::min(C, 16); ++ns) {
+                    const int cps = (C + ns - 1) / ns, ns_eff = (C + cps - 1) / cps;
+                    const long long waves = ((long long)bt * tt_ * ns_eff + slots - 1) / slots;
+                    const double cost = (double)waves * ((double)cps * unit + 4.5 * (t == 32 ? 1.0 : 8.0 / 5.0 * 0.75));
+                    if (best < 0 || cost < best) {
+                        best = cost;
+                        n_split = ns_eff;
+                        tr = t;
+                    }
                 }
             }
         }
 #ifdef CHIME_DD_SWEEP
         if (getenv("DD_SPLIT")) n_split = atoi(getenv("DD_SPLIT"));
+        if (getenv("DD_TR")) tr = atoi(getenv("DD_TR"));
 #endif
+        const int tt = (n_out + tr - 1) / tr;
         dp.c_per_split = (C + n_split - 1) / n_split;
         n_split = (C + dp.c_per_split - 1) / dp.c_per_split;
         if (n_split > 1) e = cudaMemsetAsync(out_u32, 0, (size_t)n_beams * n_out * sizeof(uint32_t), st);
         if (e == cudaSuccess) {
             dim3 grid(bt, tt, n_split);
-            if (n_beams == 1024) chime_dd::dedisperse_kernel<1024><<<grid, chime_dd::kThreads, 0, st>>>(dp);
-            else chime_dd::dedisperse_kernel<0><<<grid, chime_dd::kThreads, 0, st>>>(dp);
+            if (n_beams == 1024 && tr == 32) chime_dd::dedisperse_kernel<1024, 32><<<grid, chime_dd::kThreads, 0, st>>>(dp);
+            else if (n_beams == 1024) chime_dd::dedisperse_kernel<1024, 16><<<grid, chime_dd::kThreads, 0, st>>>(dp);
+            else if (tr == 32) chime_dd::dedisperse_kernel<0, 32><<<grid, chime_dd::kThreads, 0, st>>>(dp);
+            else chime_dd::dedisperse_kernel<0, 16><<<grid, chime_dd::kThreads, 0, st>>>(dp);
             e = cudaGetLastError();
         }
     }

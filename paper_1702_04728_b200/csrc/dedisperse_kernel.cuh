@@ -33,16 +33,18 @@ struct Params {
 // NB = beams in the array as a compile-time constant (1024: the full array), or 0 = p.n_beams at run time (beam shards).
 // With a constant the 32 loads of a pass are one base register + immediate offsets; with a run-time stride each load
 // needs its own 64-bit address (100 registers instead of 90, 0.203 ms instead of 0.156 ms on the bench workload).
-template <int NB>
-__global__ void __launch_bounds__(kThreads, 4) dedisperse_kernel(const Params p) {
+// TR = output samples per thread: 32 (TR), or 16 for short outputs, where 32-sample tiles would leave most of the SMs
+// idle or force a deep channel split (twice the CTAs, 8 resident per SM instead of 5).
+template <int NB, int TR>
+__global__ void __launch_bounds__(kThreads, (TR == 32 ? 4 : 8)) dedisperse_kernel(const Params p) {
     const int tid = threadIdx.x;
     const int q = tid & 3;
     const int b = blockIdx.x * kBeamsPerCta + (tid >> 2);
-    const int r0 = blockIdx.y * kTR;
-    uint32_t acc[kTR];
+    const int r0 = blockIdx.y * TR;
+    uint32_t acc[TR];
 #pragma unroll
-    for (int r = 0; r < kTR; ++r) acc[r] = 0u;
-    const int n_valid = min(kTR, p.n_out - r0);      // ragged last tile
+    for (int r = 0; r < TR; ++r) acc[r] = 0u;
+    const int n_valid = min(TR, p.n_out - r0);      // ragged last tile
     const size_t frame_words = NB ? (size_t)NB * 4 : (size_t)p.n_beams * 4;
     const int c_lo = blockIdx.z * p.c_per_split, c_hi = min(p.C, c_lo + p.c_per_split);
     int4 dl_next = *reinterpret_cast<const int4 *>(p.delay + c_lo * 16 + 4 * q);
@@ -61,22 +63,22 @@ __global__ void __launch_bounds__(kThreads, 4) dedisperse_kernel(const Params p)
                                   (dl.w == v ? 0x01000000u : 0u);
             if (mask == 0u) continue;
             const uint32_t *src = base + (size_t)(r0 + v) * frame_words;
-            uint32_t w[kTR];   // all TR loads are issued before the first use: 32 x 128 B per warp in flight
+            uint32_t w[TR];   // all TR loads are issued before the first use: 32 x 128 B per warp in flight
 #pragma unroll
-            for (int r = 0; r < kTR; ++r) w[r] = (r < n_valid) ? __ldg(src + (size_t)r * frame_words) : 0u;
+            for (int r = 0; r < TR; ++r) w[r] = (r < n_valid) ? __ldg(src + (size_t)r * frame_words) : 0u;
 #pragma unroll
-            for (int r = 0; r < kTR; ++r) acc[r] = __dp4a(w[r], mask, acc[r]);
+            for (int r = 0; r < TR; ++r) acc[r] = __dp4a(w[r], mask, acc[r]);
         }
     }
     // sum the 4 quads of a beam (lanes 4k .. 4k+3), then lane q == 0 .. 3 stores every 4th sample
 #pragma unroll
-    for (int r = 0; r < kTR; ++r) {
+    for (int r = 0; r < TR; ++r) {
         acc[r] += __shfl_xor_sync(0xFFFFFFFFu, acc[r], 1);
         acc[r] += __shfl_xor_sync(0xFFFFFFFFu, acc[r], 2);
     }
     uint32_t *dst = p.out + (size_t)b * p.n_out + r0;
 #pragma unroll
-    for (int r = 0; r < kTR; ++r)
+    for (int r = 0; r < TR; ++r)
         if ((r & 3) == q && r < n_valid) {
             if (gridDim.z == 1) dst[r] = acc[r];
             else atomicAdd(dst + r, acc[r]);
