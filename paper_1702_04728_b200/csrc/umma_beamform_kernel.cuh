@@ -157,12 +157,6 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo, uint
     return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) |
            ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | (1ull << 46);
 }
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t *v) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                 : "r"(taddr) : "memory");
-}
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t *v) {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
                  "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
@@ -250,15 +244,18 @@ __device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned cha
     }
 }
 
-// ---- accumulator drain: one digit pass (64 s32 columns of this thread's lane) folded into 64 fp32 partial sums ------
-// |a| < 2^22 (K 512 x 128 x 64), so the integer a + 0x4B400000 IS the bit pattern of the float M + a, M = 1.5 * 2^23
-// (exact): the conversion is one integer add (ALU pipe), and y = a2 + a1 / 256 + a0 / 65536 in units of the top digit
-// costs one more FP32 instruction per value and pass.  Column 32 part + j (part 0 = real, 1 = imaginary, j = 16 set +
-// u') goes to y[2 j + part], so that (re, im) pairs and the 16-byte groups the sender stores sit in consecutive
-// registers.  The hand-back of the slot is the critical path of the whole pipeline (two 64-column slots rotate under
-// three digit passes), so it happens as soon as the columns are in registers, BEFORE the arithmetic.
-constexpr uint32_t kMagicBits = 0x4B400000u;               // 1.5 * 2^23 = 12582912
-constexpr float kMagicSum = 12582912.0f + 49152.0f + 192.0f;   // M (1 + 2^-8 + 2^-16), an exact integer < 2^24
+// ---- accumulator drain: one digit pass (64 s32 columns of this thread's lane) folded into 64 partial sums ------------
+// The three digit sums are recombined in INTEGER arithmetic: |a_p| < 2^22 (K 512 x 128 x 64), so u = 256 a2 + a1 fits in
+// 31 bits (one shift-add on the ALU pipe), and v = u + floor(a0 / 256) (one more) is the sum in units of the MIDDLE digit
+// with the last digit's fraction dropped: an error below one unit on values of ~5e6, i.e. 2e-7, far inside the weights'
+// own 24-bit rounding.  Pass 0 costs no instruction at all (the loaded columns ARE the partial sums), and the only
+// conversion is one cvt.rn.f32.s32 per value after pass 2.  (Before: fp32 recombination a2 + a1 / 256 + a0 / 65536 with a
+// magic-constant conversion per pass, 6 instructions per value instead of 3.)  The factor 256^2 on the intensities is
+// taken out at the frame end.  Column 32 part + j (part 0 = real, 1 = imaginary, j = 16 set + u') goes to y[2 j + part],
+// so that (re, im) pairs and the 16-byte groups the sender stores sit in consecutive registers.  The hand-back of the slot
+// is the critical path of the whole pipeline (two 64-column slots rotate under three digit passes), so it happens as soon
+// as the columns are in registers, BEFORE the arithmetic.
+constexpr float kMidDigitUnits2 = 1.0f / 65536.0f;         // y is in units of the middle digit: intensities x 256^2
 
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t *v) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -290,34 +287,56 @@ __device__ __forceinline__ void slot_release(const uint32_t slot, const int lane
     asm volatile("bar.arrive %0, %1;" :: "r"(2 + slot), "n"(kSlotBarThreads) : "memory");
 }
 
-// W = columns per load: 32 (two round trips per pass; 64 + 32 registers at the drain's 112) or 16 (four round trips).
-// ptxas may still issue several loads before the arithmetic of the first and spill partial sums for it: W = 16 made
-// that worse, not better (measured on the U = 256 instantiation), so both run W = 32.
-template <int P, int W>
-__device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64], const uint32_t slot, const int lane, long long *t_rel = nullptr) {
-    constexpr float kS = P == 1 ? 1.0f / 256.0f : 1.0f / 65536.0f;
-#pragma unroll
-    for (int c = 0; c < 64 / W; ++c) {   // columns W c .. W c + W - 1: part = column / 32, j = column % 32
-        uint32_t h[W];
-        if constexpr (W == 32) tmem_ld32(tslot + W * c, h);
-        else tmem_ld16(tslot + W * c, h);
+// The same load with its 32 destination registers 2 apart (columns of one part -> y[2 j + part]): pass 0 loads straight
+// into the partial sums, both halves in flight under ONE wait.
+#define Y2(i) "=r"(y[2 * (i) + PART])
+template <int PART>
+__device__ __forceinline__ void tmem_ld32_strided(uint32_t taddr, uint32_t (&y)[64]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                 "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+                 "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                 : Y2(0), Y2(1), Y2(2), Y2(3), Y2(4), Y2(5), Y2(6), Y2(7), Y2(8), Y2(9), Y2(10), Y2(11), Y2(12), Y2(13), Y2(14), Y2(15),
+                   Y2(16), Y2(17), Y2(18), Y2(19), Y2(20), Y2(21), Y2(22), Y2(23), Y2(24), Y2(25), Y2(26), Y2(27), Y2(28), Y2(29), Y2(30), Y2(31)
+                 : "r"(taddr) : "memory");
+}
+#undef Y2
+
+// y: the 64 partial sums of this thread's beam as s32 bit patterns (passes 0, 1) / fp32 bit patterns (after pass 2).
+template <int P>
+__device__ __forceinline__ void drain_pass(const uint32_t tslot, uint32_t (&y)[64], const uint32_t slot, const int lane, long long *t_rel = nullptr) {
+    if constexpr (P == 0) {
+        tmem_ld32_strided<0>(tslot, y);
+        tmem_ld32_strided<1>(tslot + 32, y);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        if (c == 64 / W - 1) {
-            slot_release(slot, lane);
+        slot_release(slot, lane);
 #ifdef CHIME_PROF
-            *t_rel = clock64();
+        *t_rel = clock64();
 #endif
-        }
+    } else {
+#pragma unroll
+        for (int part = 0; part < 2; ++part) {   // columns 32 part .. 32 part + 31
+            uint32_t h[32];
+            tmem_ld32(tslot + 32 * part, h);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (part == 1) {
+                slot_release(slot, lane);
+#ifdef CHIME_PROF
+                *t_rel = clock64();
+#endif
+            }
 #if defined(CHIME_SKIP) && (CHIME_SKIP & 4)
-        y[c] = __uint_as_float(h[0] ^ h[W - 1]);
-        if (lane > 32)
+            y[part] = h[0] ^ h[31];
+            if (lane > 32)
 #endif
 #pragma unroll
-        for (int i = 0; i < W; ++i) {
-            const int col = W * c + i, part = col >> 5, j = col & 31;
-            const float f = __uint_as_float(h[i] + kMagicBits);   // (cvt.rn.f32.s32 instead: 5 % slower, measured)
-            if constexpr (P == 0) y[2 * j + part] = f - kMagicSum;
-            else y[2 * j + part] = fmaf(f, kS, y[2 * j + part]);
+            for (int j = 0; j < 32; ++j) {
+                if constexpr (P == 1) {
+                    y[2 * j + part] = (y[2 * j + part] << 8) + h[j];                        // 256 a2 + a1
+                } else {
+                    const int v = (int)y[2 * j + part] + ((int)h[j] >> 8);                  // + floor(a0 / 256)
+                    y[2 * j + part] = __float_as_uint((float)v);
+                }
+            }
         }
     }
 }
@@ -331,11 +350,10 @@ __device__ __forceinline__ void drain_pass(const uint32_t tslot, float (&y)[64],
 // Group g takes the tiles tau = 2 k + g: its passes use slots g, g ^ 1, g, so tile k is uses 2 k, 2 k + 1 of barrier
 // ACC_FULL[g][g] and use k of ACC_FULL[g][g ^ 1]: the parities are 0, k & 1, 1 -- no counters.  Everything that is only
 // needed after the three passes (destination addresses) is computed there: the drain runs at the edge of its registers.
-template <int W>
 __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const uint32_t bar0, const uint32_t recv0, const uint32_t g,
                                          const uint32_t q, const uint32_t tau, const int cyl, const int lane, const Params &prm,
                                          long long *prof_w) {
-    float y[64];
+    uint32_t y[64];
     const uint32_t tlane = tb + ((32u * q) << 16), bar_full0 = bar0 + 8u * (B_ACC_FULL + 2 * g);
 #pragma unroll
     for (int p = 0; p < 3; ++p) {
@@ -349,24 +367,24 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const 
 #endif
 #ifdef CHIME_PROF
         long long _t1 = 0;
-        if (p == 0) drain_pass<0, W>(tslot, y, slot, lane, &_t1);
-        else if (p == 1) drain_pass<1, W>(tslot, y, slot, lane, &_t1);
-        else drain_pass<2, W>(tslot, y, slot, lane, &_t1);
+        if (p == 0) drain_pass<0>(tslot, y, slot, lane, &_t1);
+        else if (p == 1) drain_pass<1>(tslot, y, slot, lane, &_t1);
+        else drain_pass<2>(tslot, y, slot, lane, &_t1);
         prof_w[6] += _t1 - _t0;
         prof_w[7] += clock64() - _t1;
 #else
-        if (p == 0) drain_pass<0, W>(tslot, y, slot, lane);
-        else if (p == 1) drain_pass<1, W>(tslot, y, slot, lane);
-        else drain_pass<2, W>(tslot, y, slot, lane);
+        if (p == 0) drain_pass<0>(tslot, y, slot, lane);
+        else if (p == 1) drain_pass<1>(tslot, y, slot, lane);
+        else drain_pass<2>(tslot, y, slot, lane);
 #endif
     }
     if (tt >= 2) {   // A_rho = E + O'/sqrt2 (set 0), A_{rho+4} = E - O'/sqrt2 (set 1)
         constexpr float s = 0.70710678118654752440f;
 #pragma unroll
         for (int k = 0; k < 32; ++k) {   // k = 2 u' + part
-            const float e = y[k], o = y[32 + k];
-            y[k] = fmaf(s, o, e);
-            y[32 + k] = fmaf(-s, o, e);
+            const float e = __uint_as_float(y[k]), o = __uint_as_float(y[32 + k]);
+            y[k] = __float_as_uint(fmaf(s, o, e));
+            y[32 + k] = __float_as_uint(fmaf(-s, o, e));
         }
     }
     const uint32_t rslot = mapa(recv0 + g * kRecvBytes, q), rbar = mapa(bar0 + 8u * (B_RECV_FULL + g), q);
@@ -379,8 +397,8 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const 
         for (int ip = 0; ip < 8; ++ip) {
             const uint32_t addr = rslot + (uint32_t)((((cyl * 2 + res) * 8 + ip) * 32 + lane) * 16);
             const int k = 32 * res + 4 * ip;
-            asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1,%2,%3,%4}, [%5];"
-                         :: "r"(addr), "f"(y[k]), "f"(y[k + 1]), "f"(y[k + 2]), "f"(y[k + 3]), "r"(rbar) : "memory");
+            asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1,%2,%3,%4}, [%5];"
+                         :: "r"(addr), "r"(y[k]), "r"(y[k + 1]), "r"(y[k + 2]), "r"(y[k + 3]), "r"(rbar) : "memory");
         }
 }
 
@@ -638,7 +656,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll 1
                 for (int t = ntiles; t > 0; --t, ++tau) {   // (tiles per frame and polarisation: a multiple of 8, so tau gives the tile type)
                     if ((tau & 1) != g) continue;
-                    epi_tile<32>(U == 128 ? (tau & 3) : ((tau >> 1) & 3), tb, bar0, recv0, g, q, tau, rank, lane, prm, prof_w);
+                    epi_tile(U == 128 ? (tau & 3) : ((tau >> 1) & 3), tb, bar0, recv0, g, q, tau, rank, lane, prm, prof_w);
                 }
             }
         }
@@ -783,7 +801,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                     float4 *scr = reinterpret_cast<float4 *>(prm.scratch + ((size_t)blockIdx.x * kMaxChunkFrames * 128 + e2 * 32 + lane) * 16);
                     uint64_t l2_keep;
                     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(l2_keep));
-                    const float nrm = prm.norm * __ldg(prm.inv_s2 + c);
+                    const float nrm = prm.norm * __ldg(prm.inv_s2 + c) * kMidDigitUnits2;
                     // ---- frame end: a9 sum of the two residue halves (+ pol 0), normalise, a10 quantise, 16-byte store per beam
                     if (res2 == 0) {
 #pragma unroll
