@@ -118,6 +118,10 @@ __device__ __forceinline__ bool mbar_try(uint32_t a, uint32_t parity) {
                  : "=r"(ok) : "r"(a), "r"(parity) : "memory");
     return ok != 0;
 }
+// Development switches (off in the product; results are WRONG with CHIME_SKIP, it is for timing only):
+//   -DCHIME_SKIP=<mask>: 1 receive side's twiddle + FFT-16 + detection, 16 its E-W phase, 2 operand preparation,
+//                        4 the drain's arithmetic, 32 the drain's tensor-memory loads;
+//   -DCHIME_PROF: clock64 around every wait of every role, read back with chime_bf_debug_prof.
 #ifdef CHIME_PROF
 __device__ long long g_prof[148 * 4][24][12];
 #define PW(code, stmt) { const long long _t = clock64(); stmt; prof_w[code] += clock64() - _t; }
@@ -305,8 +309,13 @@ __device__ __forceinline__ void tmem_ld32_strided(uint32_t taddr, uint32_t (&y)[
 template <int P>
 __device__ __forceinline__ void drain_pass(const uint32_t tslot, uint32_t (&y)[64], const uint32_t slot, const int lane, long long *t_rel = nullptr) {
     if constexpr (P == 0) {
-        tmem_ld32_strided<0>(tslot, y);
-        tmem_ld32_strided<1>(tslot + 32, y);
+#if defined(CHIME_SKIP) && (CHIME_SKIP & 32)
+        if (lane > 32)
+#endif
+        {
+            tmem_ld32_strided<0>(tslot, y);
+            tmem_ld32_strided<1>(tslot + 32, y);
+        }
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
         slot_release(slot, lane);
 #ifdef CHIME_PROF
@@ -316,6 +325,9 @@ __device__ __forceinline__ void drain_pass(const uint32_t tslot, uint32_t (&y)[6
 #pragma unroll
         for (int part = 0; part < 2; ++part) {   // columns 32 part .. 32 part + 31
             uint32_t h[32];
+#if defined(CHIME_SKIP) && (CHIME_SKIP & 32)
+            if (lane > 32)
+#endif
             tmem_ld32(tslot + 32 * part, h);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             if (part == 1) {
@@ -690,7 +702,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                         PW(10, mbar_wait(BAR(B_RECV_FULL + s), (tau >> 1) & 1, prm, 10, tau);)
                         if (rw == 0 && lane == 0) mbar_expect_tx(BAR(B_RECV_FULL + s), kRecvBytes);   // arm the slot's next tile
                         unsigned char *slot = smem + kOfsRecv + s * kRecvBytes + lane * 16;
-#if defined(CHIME_SKIP) && (CHIME_SKIP & 1)
+#if defined(CHIME_SKIP) && (CHIME_SKIP & 16)
                         if (prm.n_time < 0)
 #endif
                         {   // ---- phase 1: (beam, u' pair = rw), both residues
@@ -722,9 +734,6 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                         }
                         if constexpr (U == 128) {
                             bar_sync_named(1, 256);
-#if defined(CHIME_SKIP) && (CHIME_SKIP & 1)
-                            if (prm.n_time < 0)
-#endif
                             {   // ---- phase 2: (beam, residue = res2, E-W beam = e2)
                                 const unsigned char *base = slot + ((e2 * 2 + res2) * 8) * 512;
                                 float2 a[16];
@@ -738,9 +747,14 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                                 // residue of (tile type, column set): {0,4}, {2,6}, {1,5}, {3,7}
                                 const int tt = t & 3;
                                 const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
+#if defined(CHIME_SKIP) && (CHIME_SKIP & 1)
+                                if (prm.n_time < 0)   // (the loads and the hand-back of the slot stay: the senders wait for it)
+#endif
+                                {
 #pragma unroll
-                                for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr[rho][u]);
-                                fft16_detect(a, acc);
+                                    for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr[rho][u]);
+                                    fft16_detect(a, acc);
+                                }
                             }
                         } else if (t & 1) {
                             // U = 256: the FFT over u' has 32 points, u' = 16 h + u'': the tile of half 0 waits (E-W summed) in

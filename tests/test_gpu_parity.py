@@ -197,6 +197,38 @@ def test_every_byte_value_including_minus_eight(bf, orc, NP):
     plan.destroy()
 
 
+@pytest.mark.parametrize("NP,U", [(512, 128), (1024, 256)])
+def test_accumulator_range_limit(bf, orc, NP, U):
+    """Largest accumulators the tensor-core path can see: every input at -8 - 8i (nibble 0, |x| largest) for whole
+    blocks, coherent over the feeds, unit gains, f = f_ref (beam 128 has the all-ones weight row).  The digit sums reach
+    their bound K x 128 x 64 < 2^22 there, on which the integer recombination 256 a2 + a1 (31 bits) of the drain
+    relies; the last block of each frame is noise so that every beam has a mean power to compare against."""
+    frame = 3 * U
+    T = 2 * frame
+    freqs = np.array([600.0])
+    hb = np.zeros((1, T, 2048), dtype=np.uint8)                      # 0x00 = -8 - 8i
+    noise = synth.noise_bytes(77, 1, T).numpy()
+    hb[0, frame - U:frame] = noise[0, :U]                            # frame 0: blocks 0, 1 coherent, block 2 noise
+    hb[0, frame:frame + U] = 0xFF                                    # frame 1: +7 + 7i, then -8 - 8i, then noise
+    hb[0, T - U:] = noise[0, U:2 * U]
+    plan = bf.plan_create_ex(1, freq_mhz=freqs, zero_pad=NP, upchan_len=U, n_time=T)
+    d_in = torch.from_numpy(hb).cuda()
+    out_f32 = plan.execute_f32(d_in)
+    torch.cuda.synchronize()
+    worst = 0.0
+    for R in range(2):
+        I, _ = orc.cell(hb[0, frame * R:frame * (R + 1)], 600.0, gains=None, np_=NP, U=U)
+        got = out_f32[0, R].cpu().numpy()
+        mean = I.mean(axis=-1, keepdims=True)
+        assert mean.min() > 0
+        worst = max(worst, float((np.abs(got - I) / mean).max()))
+    # the zenith beam holds the coherent power: (2 blocks x U samples) x |2048 x 8 sqrt2|^2 / (1024 U) spread over nothing
+    assert float(out_f32[0, 0, :, 128].max()) > 1e5
+    assert worst <= REL_TOL, f"float intensities off by {worst:.3e} of the beam mean power"
+    print(f"NP={NP} U={U} accumulator range limit: worst rel err {worst:.2e}")
+    plan.destroy()
+
+
 @pytest.mark.parametrize("amp", [1e-4, 1.0, 1e3])
 def test_gain_range(bf, orc, amp):
     """Gains far from unity (the weights are scaled per channel, so only the RATIO of gains inside a channel costs
