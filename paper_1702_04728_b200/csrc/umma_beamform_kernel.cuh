@@ -15,7 +15,8 @@
 //      Weights = round(S_c * value) as 24-bit integers split into THREE balanced signed 8-bit digits (16 bits fail the
 //      1e-4 parity bar on configs[0]) that stay resident in TENSOR MEMORY (128 lanes = 128 beams,
 //      3 x 128 columns = K 512 x 3 digits); the data columns are signed bytes in shared memory; one s32 accumulator
-//      pass per digit, recombined in fp32 as a2 + a1 / 256 + a0 / 65536.  Real and imaginary outputs of a beam come
+//      pass per digit, recombined in integer arithmetic as 256 a2 + a1 + floor(a0 / 256) and converted to fp32 once
+//      (drain_pass).  Real and imaginary outputs of a beam come
 //      from the SAME weight row [Wr | -Wi] applied to two variants of the data column, [re | im] and [im | -re], so
 //      both land in the same TMEM lane (= thread) in different columns.
 //   3. E-W: Z_e = sum_cyl beta_e^cyl S_cyl (Horner), after an all-to-all by beam quarter over DSMEM: CTA r of the
