@@ -142,8 +142,10 @@ int chime_bf_update_pointings(chime_bf_plan *plan, void *cuda_stream, double f_r
  * chime_bf_dedisp_delays: HOST host_out [C][16] int32 (may be NULL) and HOST *n_out (may be NULL).
  * chime_bf_dedisperse:    DEVICE beams_u8 [C][n_frames][1024][16] (the layout execute writes), 16-byte aligned;
  *                         DEVICE out_u32 [1024][n_out]; n_out must be the value dedisp_delays reports (>= 1).
- *                         Asynchronous on cuda_stream; one kernel launch; uses a plan-owned 64*C-byte table, so
- *                         one dedisperse call per plan may be in flight at a time.
+ *                         Asynchronous on cuda_stream; one kernel launch, preceded by a small clearing kernel when
+ *                         the channel loop is split over CTAs, and by the upload of the delay table unless the
+ *                         calling thread's previous call left the same table in the same place on the same stream;
+ *                         uses a plan-owned 64*C-byte table, so one dedisperse call per plan may be in flight at a time.
  */
 int chime_bf_dedisp_delays(const chime_bf_plan *plan, double dm, double f_ref_mhz, int32_t *host_out,
                            int *n_out);
@@ -184,12 +186,13 @@ int chime_bf_dedisperse_beams(void *cuda_stream, const uint8_t *beams_u8, int n_
  * instead of a caller-owned buffer.  Limit: n_coarse <= CHIME_BF_NOALLOC_MAX_COARSE (1024 = the full band; the array is
  * 64 KiB and every GPU that loads the library holds it until exit); a larger n_coarse is CHIME_BF_E_INVALID_ARG with a
  * message.  The call allocates nothing on the device and frees nothing (no cudaMalloc / cudaFree / allocating library
- * routine; on the host one thread-local table is sized on a thread's first call).  Arguments as
+ * routine; on the host two thread-local tables are sized on a thread's first calls).  Arguments as
  * chime_bf_dedisperse_beams without delay_scratch: beams_u8, out_u32 DEVICE and caller-owned; freq_mhz HOST.
  * Every call on a device shares the one array and finds the previous call's table in it: each call rewrites the
- * n_coarse*16 entries it uses on `cuda_stream` before its kernel reads them (and clears out_u32 when the channel loop
- * is split), so calls that follow each other on one stream are safe; calls that OVERLAP on the GPU (different streams
- * without an event between them) race on the table.
+ * n_coarse*16 entries it uses on `cuda_stream` before its kernel reads them (left out only when the calling thread's
+ * previous call wrote exactly this table, on this stream, and no other call has written the array since; out_u32 is
+ * cleared when the channel loop is split), so calls that follow each other on one stream are safe; calls that OVERLAP
+ * on the GPU (different streams without an event between them) race on the table.
  */
 #define CHIME_BF_NOALLOC_MAX_COARSE 1024
 int chime_bf_dedisperse_beams_noalloc(void *cuda_stream, const uint8_t *beams_u8, int n_coarse, const double *freq_mhz,

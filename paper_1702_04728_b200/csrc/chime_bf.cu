@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "beam_major.cuh"
+#include <atomic>
 #include "dedisperse_kernel.cuh"
 #include "fp32_peak.cuh"
 #include "umma_beamform_kernel.cuh"
@@ -398,10 +399,33 @@ int32_t *noalloc_delay_table() {
     return ptr[dev];
 }
 
+// Bumped by every upload of a delay table and by chime_bf_destroy (a new plan may get a freed plan's address).
+static std::atomic<unsigned long long> g_dd_upload_epoch{0};
+
+// lib_owned: d_delay is written by this function only (a plan's table, the built-in array of the no-alloc call), so an
+// upload of the same table to the same place on the same stream can be left out.  A caller's scratch is always rewritten.
 int launch_dedisperse(void *stream, const uint8_t *beams_u8, int C, int R, int n_beams, const std::vector<int32_t> &tab,
-                      int32_t *d_delay, uint32_t *out_u32, int n_out) {
+                      int32_t *d_delay, uint32_t *out_u32, int n_out, bool lib_owned) {
     cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = cudaMemcpyAsync(d_delay, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+    // The table goes up only when it differs from what this thread last put into this device array on this stream (the
+    // usual caller dedisperses buffer after buffer to the same DM): one stream operation less in front of a kernel that
+    // takes 40 - 140 us.  A different stream, array or table uploads again; so does any other writer of the array in
+    // between, because every such writer is a call of this function and replaces the record.
+    struct Uploaded { const int32_t *dst = nullptr; cudaStream_t st = nullptr; int dev = -1; std::vector<int32_t> tab; };
+    static thread_local Uploaded last;
+    static thread_local unsigned long long my_epoch = 0;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    const bool same = lib_owned && e == cudaSuccess && last.dst == d_delay && last.st == st && last.dev == dev &&
+                      my_epoch == g_dd_upload_epoch.load() && last.tab == tab;
+    if (e == cudaSuccess && !same) {
+        e = cudaMemcpyAsync(d_delay, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+        last.dst = d_delay;
+        last.st = st;
+        last.dev = dev;
+        last.tab = tab;
+        my_epoch = ++g_dd_upload_epoch;
+    }
     if (e == cudaSuccess) {
         chime_dd::Params dp;
         dp.in = reinterpret_cast<const uint32_t *>(beams_u8);
@@ -443,14 +467,33 @@ int launch_dedisperse(void *stream, const uint8_t *beams_u8, int C, int R, int n
         const int tt = (n_out + tr - 1) / tr;
         dp.c_per_split = (C + n_split - 1) / n_split;
         n_split = (C + dp.c_per_split - 1) / dp.c_per_split;
-        if (n_split > 1) e = cudaMemsetAsync(out_u32, 0, (size_t)n_beams * n_out * sizeof(uint32_t), st);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(bt, tt, n_split);
+        cfg.blockDim = dim3(chime_dd::kThreads);
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        if (n_split > 1) {
+            // split channel loop: clear the output with a kernel and let the dedispersion start under it (it waits for
+            // the clearing only before its atomics, see dedisperse_kernel)
+            const size_t n_words = (size_t)n_beams * n_out, head = std::min<size_t>(n_words, (4 - (((uintptr_t)out_u32 >> 2) & 3)) & 3);
+            const size_t n16 = (n_words - head) / 4, tail = n_words - head - 4 * n16;
+            if (head) e = cudaMemsetAsync(out_u32, 0, head * sizeof(uint32_t), st);   // (only for an output that is not 16-byte aligned)
+            if (e == cudaSuccess) {
+                const int zb = (int)std::min<size_t>((n16 + 255) / 256 + 1, 148 * 4);
+                chime_dd::zero_kernel<<<zb, 256, 0, st>>>(reinterpret_cast<uint4 *>(out_u32 + head), n16, out_u32 + head + 4 * n16, (int)tail);
+                e = cudaGetLastError();
+            }
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+        }
         if (e == cudaSuccess) {
-            dim3 grid(bt, tt, n_split);
-            if (n_beams == 1024 && tr == 32) chime_dd::dedisperse_kernel<1024, 32><<<grid, chime_dd::kThreads, 0, st>>>(dp);
-            else if (n_beams == 1024) chime_dd::dedisperse_kernel<1024, 16><<<grid, chime_dd::kThreads, 0, st>>>(dp);
-            else if (tr == 32) chime_dd::dedisperse_kernel<0, 32><<<grid, chime_dd::kThreads, 0, st>>>(dp);
-            else chime_dd::dedisperse_kernel<0, 16><<<grid, chime_dd::kThreads, 0, st>>>(dp);
-            e = cudaGetLastError();
+            if (n_beams == 1024 && tr == 32) e = cudaLaunchKernelEx(&cfg, chime_dd::dedisperse_kernel<1024, 32>, dp);
+            else if (n_beams == 1024) e = cudaLaunchKernelEx(&cfg, chime_dd::dedisperse_kernel<1024, 16>, dp);
+            else if (tr == 32) e = cudaLaunchKernelEx(&cfg, chime_dd::dedisperse_kernel<0, 32>, dp);
+            else e = cudaLaunchKernelEx(&cfg, chime_dd::dedisperse_kernel<0, 16>, dp);
+            if (e == cudaSuccess) e = cudaGetLastError();
         }
     }
     if (e != cudaSuccess) { set_err("dedisperse: %s", cudaGetErrorString(e)); return CHIME_BF_E_CUDA; }
@@ -725,7 +768,7 @@ int chime_bf_dedisperse(chime_bf_plan *pl, void *stream, const uint8_t *beams_u8
         set_err("dedisperse: n_out must be n_frames - max delay = %d (got %d)", n_full, n_out);
         return CHIME_BF_E_INVALID_ARG;
     }
-    return launch_dedisperse(stream, beams_u8, pl->C, pl->R, 1024, tab, pl->d_delay, out_u32, n_out);
+    return launch_dedisperse(stream, beams_u8, pl->C, pl->R, 1024, tab, pl->d_delay, out_u32, n_out, true);
 }
 
 int chime_bf_dedisperse_stream_begin(chime_bf_plan *pl, void *stream, double dm, double f_ref_mhz, int *max_delay) {
@@ -819,7 +862,7 @@ int chime_bf_dedisperse_beams(void *stream, const uint8_t *beams_u8, int n_coars
         set_err("dedisperse_beams: n_out must be n_frames - max delay = %d (got %d)", n_frames - mx, n_out);
         return CHIME_BF_E_INVALID_ARG;
     }
-    return launch_dedisperse(stream, beams_u8, n_coarse, n_frames, n_beams, tab, delay_scratch, out_u32, n_out);
+    return launch_dedisperse(stream, beams_u8, n_coarse, n_frames, n_beams, tab, delay_scratch, out_u32, n_out, false);
 }
 
 int chime_bf_dedisperse_beams_noalloc(void *stream, const uint8_t *beams_u8, int n_coarse, const double *freq_mhz,
@@ -850,9 +893,10 @@ int chime_bf_dedisperse_beams_noalloc(void *stream, const uint8_t *beams_u8, int
     }
     int32_t *d_delay = noalloc_delay_table();   // the device address of the array on the current device
     if (d_delay == nullptr) return CHIME_BF_E_CUDA;
-    // launch_dedisperse rewrites tab.size() entries of the table on `stream` before the kernel reads them, and clears
-    // out_u32 when the channel loop is split: nothing of the previous call's contents is read.
-    return launch_dedisperse(stream, beams_u8, n_coarse, n_frames, n_beams, tab, d_delay, out_u32, n_out);
+    // launch_dedisperse rewrites tab.size() entries of the table on `stream` before the kernel reads them (unless this
+    // thread's previous call left exactly this table there, on this stream), and clears out_u32 when the channel loop is
+    // split: nothing else of a previous call's contents is read.
+    return launch_dedisperse(stream, beams_u8, n_coarse, n_frames, n_beams, tab, d_delay, out_u32, n_out, true);
 }
 
 int chime_bf_get_ns_index(const chime_bf_plan *plan, int32_t *host_out) {
@@ -939,6 +983,7 @@ void chime_bf_destroy(chime_bf_plan *pl) {
     if (!pl) return;
     cudaFree(pl->d_stage_in);
     cudaFree(pl->d_stage_out);
+    ++g_dd_upload_epoch;   // no later plan that gets this address may be taken for this one (launch_dedisperse)
     cudaFree(pl->d_delay);
     cudaFree(pl->d_ring);
     cudaFree(pl->d_delay_stream);

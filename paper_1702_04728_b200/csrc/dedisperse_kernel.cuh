@@ -77,12 +77,25 @@ __global__ void __launch_bounds__(kThreads, (TR == 32 ? 4 : 8)) dedisperse_kerne
         acc[r] += __shfl_xor_sync(0xFFFFFFFFu, acc[r], 2);
     }
     uint32_t *dst = p.out + (size_t)b * p.n_out + r0;
+    // Split channel loop: the output is cleared by zero_kernel, the launch before this one in the stream.  This kernel
+    // is launched with programmatic stream serialization, so it starts (and does all of its loads) while the clearing
+    // still runs; only here, before the first atomic, does it wait for that grid to be complete and visible.
+    if (gridDim.z > 1) asm volatile("griddepcontrol.wait;" ::: "memory");
 #pragma unroll
     for (int r = 0; r < TR; ++r)
         if ((r & 3) == q && r < n_valid) {
             if (gridDim.z == 1) dst[r] = acc[r];
             else atomicAdd(dst + r, acc[r]);
         }
+}
+
+// Clears the output of a split launch (instead of a memset node: a kernel can be the primary of a programmatic
+// dependent launch).  Lets the dependent grid start at once.
+__global__ void __launch_bounds__(256) zero_kernel(uint4 *out, size_t n16, uint32_t *tail, int n_tail) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) out[i] = make_uint4(0u, 0u, 0u, 0u);
+    if (blockIdx.x == 0 && threadIdx.x < n_tail) tail[threadIdx.x] = 0u;
 }
 
 // ---- streaming form: sweeps longer than one execute buffer (PAPER.md:86 asks for a HIGH nominal DM) ------------------

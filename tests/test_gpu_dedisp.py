@@ -43,6 +43,46 @@ def test_dedisperse_bit_exact(bf, orc, C, R, U, dm, step):
     plan.destroy()
 
 
+def test_repeated_calls_reuse_the_uploaded_table_and_stay_exact(bf, orc):
+    """A call leaves the delay-table upload out when the calling thread's previous call put the same table into the same
+    library-owned array on the same stream.  Sequences that must all stay bit-exact against the oracle: the same DM twice
+    (second upload left out), another DM (uploaded), the first one again; the no-alloc array the same way, with a call
+    on ANOTHER stream and a call of another shape in between; a plan destroyed and re-created (possibly at the same address)."""
+    C, R, U = 6, 120, 128
+    freqs = synth.chime_freqs_mhz(C, 100)
+    g = torch.Generator(device="cuda").manual_seed(synth.BASE_SEED + 99)
+    beams = torch.randint(0, 256, (C, R, 4, 256, 16), dtype=torch.uint8, device="cuda", generator=g)
+    hb = beams.cpu().numpy().reshape(C, R, 1024, 16)[:, :, ::37, :]        # 28 of the 1024 beams for the oracle
+    want = {}
+    for dm in (5.0, 8.0):
+        tab, _ = orc.dedisp_delays(freqs, dm, U=U)
+        want[dm] = orc.dedisperse(hb, tab)
+
+    def check(out, dm):
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy()[::37].astype(np.int64), want[dm]), dm
+
+    for rep in range(2):      # second round: a new plan, maybe at the freed plan's addresses
+        plan = bf.plan_create_ex(C, freq_mhz=freqs, upchan_len=U, n_time=R * 3 * U)
+        for dm in (5.0, 5.0, 8.0, 5.0, 5.0):
+            check(plan.dedisperse(beams, dm), dm)
+        plan.destroy()
+    b4 = beams.reshape(C, R, 1024, 16)
+    side = torch.cuda.Stream()
+    for dm, stream in ((5.0, None), (5.0, None), (8.0, None), (8.0, side), (8.0, None), (5.0, side), (5.0, side)):
+        _, mx = bf.dedisp_delays_ex(freqs, dm)
+        out = torch.full((1024, R - mx), -7, dtype=torch.int32, device="cuda")
+        torch.cuda.synchronize()
+        bf.dedisperse_beams_noalloc(b4, freqs, dm, out, stream=stream)
+        check(out, dm)
+        if dm == 8.0 and stream is None:      # another shape through the same array in between
+            small = torch.randint(0, 256, (3, 40, 32, 16), dtype=torch.uint8, device="cuda")
+            o2 = torch.empty((32, 40), dtype=torch.int32, device="cuda")
+            bf.dedisperse_beams_noalloc(small, synth.chime_freqs_mhz(3, 7), 0.0, o2)
+            torch.cuda.synchronize()
+            assert torch.equal(o2, small.to(torch.int32).sum(dim=(0, 3)).transpose(0, 1).contiguous())
+
+
 def test_sweep_longer_than_buffer_is_an_error(bf):
     plan = bf.plan_create_ex(2, freq_mhz=[800.0, 400.390625], n_time=10 * 384)
     _, n_out = plan.dedisp_delays(500.0)
