@@ -363,6 +363,7 @@ __device__ __forceinline__ void drain_pass(const uint32_t tslot, uint32_t (&y)[6
 // Group g takes the tiles tau = 2 k + g: its passes use slots g, g ^ 1, g, so tile k is uses 2 k, 2 k + 1 of barrier
 // ACC_FULL[g][g] and use k of ACC_FULL[g][g ^ 1]: the parities are 0, k & 1, 1 -- no counters.  Everything that is only
 // needed after the three passes (destination addresses) is computed there: the drain runs at the edge of its registers.
+template <bool DRAIN_FFT>
 __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const uint32_t bar0, const uint32_t recv0, const uint32_t g,
                                          const uint32_t q, const uint32_t tau, const int cyl, const int lane, const Params &prm,
                                          long long *prof_w) {
@@ -400,6 +401,29 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const 
             y[32 + k] = __float_as_uint(fmaf(-s, o, e));
         }
     }
+    if constexpr (DRAIN_FFT) {
+        // upchan 128: the rest of the time transform (twiddle W_128^{rho u'}, FFT-16 over u') runs HERE, on the 2 x 16
+        // values of this thread's beam that are in registers anyway, before the E-W sum instead of after it (both are
+        // linear and act on different axes).  The receive side is then one phase -- E-W sum per frequency bin, |.|^2 --
+        // with no write-back, no re-read and no barrier per tile: a third of its shared-memory traffic, on the pipe
+        // that the tensor core's operand reads share.  Position i of a set afterwards holds bin
+        // bitrev(i) of the 16-point transform.
+#pragma unroll
+        for (int set = 0; set < 2; ++set) {
+            const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * set;      // residues {0,4}, {2,6}, {1,5}, {3,7} by tile type
+            float2 a[16];
+#pragma unroll
+            for (int u = 0; u < 16; ++u) a[u] = make_float2(__uint_as_float(y[32 * set + 2 * u]), __uint_as_float(y[32 * set + 2 * u + 1]));
+#pragma unroll
+            for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr[rho][u]);
+            fft_dif<16>(a);
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                y[32 * set + 2 * u] = __float_as_uint(a[u].x);
+                y[32 * set + 2 * u + 1] = __float_as_uint(a[u].y);
+            }
+        }
+    }
     const uint32_t rslot = mapa(recv0 + g * kRecvBytes, q), rbar = mapa(bar0 + 8u * (B_RECV_FULL + g), q);
     PW(5, mbar_wait(bar0 + 8u * (B_SLOT_FREE + 2 * q + g), ((tau >> 1) & 1) ^ 1, prm, 5);)     // the destination has consumed this slot's previous tile
     // Asynchronous stores: each reports its 16 bytes to the destination's mbarrier (complete_tx), so the receiver's
@@ -429,6 +453,22 @@ __device__ __forceinline__ void slot_free_arrive(const float2 (&a)[16], const ui
                  : "r"(__float_as_uint(a[1].y)), "r"(__float_as_uint(a[3].y)), "r"(__float_as_uint(a[5].y)),
                    "r"(__float_as_uint(a[7].y)), "r"(__float_as_uint(a[9].y)), "r"(__float_as_uint(a[11].y)),
                    "r"(__float_as_uint(a[13].y)), "r"(__float_as_uint(a[15].y)));
+    dep = __reduce_or_sync(0xffffffffu, dep);   // every lane's loads
+    if (lane == 0 && dep != 0) {
+#pragma unroll
+        for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(mapa(sf_local, sc));
+    }
+}
+// (upchan 128: the 8 sixteen-byte loads of the single receive phase)
+__device__ __forceinline__ void slot_free_arrive(const float4 (&v)[2][4], const uint32_t sf_local, const int lane) {
+    uint32_t dep;
+    asm volatile("{ .reg .b32 t0, t1;\n or.b32 t0, %1, %2;\n or.b32 t1, %3, %4;\n or.b32 t0, t0, t1;\n"
+                 " or.b32 t1, %5, %6;\n or.b32 t0, t0, t1;\n or.b32 t1, %7, %8;\n or.b32 t0, t0, t1;\n"
+                 " or.b32 %0, t0, 1; }"
+                 : "=r"(dep)
+                 : "r"(__float_as_uint(v[0][0].w)), "r"(__float_as_uint(v[0][1].w)), "r"(__float_as_uint(v[0][2].w)),
+                   "r"(__float_as_uint(v[0][3].w)), "r"(__float_as_uint(v[1][0].w)), "r"(__float_as_uint(v[1][1].w)),
+                   "r"(__float_as_uint(v[1][2].w)), "r"(__float_as_uint(v[1][3].w)));
     dep = __reduce_or_sync(0xffffffffu, dep);   // every lane's loads
     if (lane == 0 && dep != 0) {
 #pragma unroll
@@ -669,7 +709,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll 1
                 for (int t = ntiles; t > 0; --t, ++tau) {   // (tiles per frame and polarisation: a multiple of 8, so tau gives the tile type)
                     if ((tau & 1) != g) continue;
-                    epi_tile(U == 128 ? (tau & 3) : ((tau >> 1) & 3), tb, bar0, recv0, g, q, tau, rank, lane, prm, prof_w);
+                    epi_tile<U == 128>(U == 128 ? (tau & 3) : ((tau >> 1) & 3), tb, bar0, recv0, g, q, tau, rank, lane, prm, prof_w);
                 }
             }
         }
@@ -683,7 +723,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         // Per frame the two residue halves meet in shared memory and the odd warps, which then hold all 16 fine channels
         // of (E-W beam, beam), park the polarisation-0 sums in a per-CTA scratch (L2) and finish the frame after pol 1.
         const int rw = warp - 16;
-        const int res2 = rw & 1, e2 = rw >> 1;
+        const int res2 = rw & 1, e2 = U == 128 ? (rw & 3) : (rw >> 1);   // upchan 128: e2 = E-W beam of the frame-end role (warps 0-3)
         const uint32_t sf0 = BAR(B_SLOT_FREE + 2 * rank);   // slot 0's barrier of this CTA's beams (in every source CTA); slot 1's is 8 bytes further
         uint32_t tau = 0;
         ITEM_LOOP
@@ -703,6 +743,41 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                         PW(10, mbar_wait(BAR(B_RECV_FULL + s), (tau >> 1) & 1, prm, 10, tau);)
                         if (rw == 0 && lane == 0) mbar_expect_tx(BAR(B_RECV_FULL + s), kRecvBytes);   // arm the slot's next tile
                         unsigned char *slot = smem + kOfsRecv + s * kRecvBytes + lane * 16;
+                        if constexpr (U == 128) {
+                            // ---- upchan 128: ONE phase.  The senders have already run the time transform (epi_tile), so cell
+                            // (cyl, res, position pair, beam) holds frequency bins: thread <-> (beam = lane, position pair = rw)
+                            // sums the 4 cylinders into the 4 E-W beams (Horner in beta_e) for both residues and adds |.|^2 to
+                            // its 4 x 2 partial intensities (positions 2 rw, 2 rw + 1 = fine channels g0, g0 + 8; both
+                            // residues of a tile belong to the same fine channel).
+                            const unsigned char *base = slot + rw * 512;
+                            float4 sv[2][4];
+#pragma unroll
+                            for (int res = 0; res < 2; ++res)
+#pragma unroll
+                                for (int cy = 0; cy < 4; ++cy)
+                                    sv[res][cy] = *reinterpret_cast<const float4 *>(base + ((cy * 2 + res) * 8) * 512);
+                            slot_free_arrive(sv, sf0 + 8 * s, lane);   // the slot is in registers: hand it back BEFORE the arithmetic
+#if defined(CHIME_SKIP) && (CHIME_SKIP & 16)
+                            if (prm.n_time < 0)
+#endif
+#pragma unroll
+                            for (int res = 0; res < 2; ++res)
+#pragma unroll
+                                for (int e = 0; e < 4; ++e) {
+                                    // Horner in beta_e: z = s0 + b (s1 + b (s2 + b s3)), two points at once
+                                    const float2 bx = make_float2(be[e].x, be[e].x), by = make_float2(-be[e].y, be[e].y);
+                                    float2 za = make_float2(sv[res][3].x, sv[res][3].y), zb = make_float2(sv[res][3].z, sv[res][3].w);
+#pragma unroll
+                                    for (int cy = 2; cy >= 0; --cy) {
+                                        const float2 sa = make_float2(sv[res][cy].x, sv[res][cy].y), sb = make_float2(sv[res][cy].z, sv[res][cy].w);
+                                        const float2 ta = __ffma2_rn(za, bx, sa), tb2 = __ffma2_rn(zb, bx, sb);
+                                        za = __ffma2_rn(make_float2(za.y, za.x), by, ta);
+                                        zb = __ffma2_rn(make_float2(zb.y, zb.x), by, tb2);
+                                    }
+                                    acc[2 * e] = fmaf(za.x, za.x, fmaf(za.y, za.y, acc[2 * e]));
+                                    acc[2 * e + 1] = fmaf(zb.x, zb.x, fmaf(zb.y, zb.y, acc[2 * e + 1]));
+                                }
+                        } else {
 #if defined(CHIME_SKIP) && (CHIME_SKIP & 16)
                         if (prm.n_time < 0)
 #endif
@@ -733,31 +808,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         }
-                        if constexpr (U == 128) {
-                            bar_sync_named(1, 256);
-                            {   // ---- phase 2: (beam, residue = res2, E-W beam = e2)
-                                const unsigned char *base = slot + ((e2 * 2 + res2) * 8) * 512;
-                                float2 a[16];
-#pragma unroll
-                                for (int k = 0; k < 8; ++k) {
-                                    const float4 v = *reinterpret_cast<const float4 *>(base + k * 512);
-                                    a[2 * k] = make_float2(v.x, v.y);
-                                    a[2 * k + 1] = make_float2(v.z, v.w);
-                                }
-                                slot_free_arrive(a, sf0 + 8 * s, lane);   // the slot is in registers: hand it back BEFORE the arithmetic
-                                // residue of (tile type, column set): {0,4}, {2,6}, {1,5}, {3,7}
-                                const int tt = t & 3;
-                                const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
-#if defined(CHIME_SKIP) && (CHIME_SKIP & 1)
-                                if (prm.n_time < 0)   // (the loads and the hand-back of the slot stay: the senders wait for it)
-#endif
-                                {
-#pragma unroll
-                                    for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr[rho][u]);
-                                    fft16_detect(a, acc);
-                                }
-                            }
-                        } else if (t & 1) {
+                        if (t & 1) {
                             // U = 256: the FFT over u' has 32 points, u' = 16 h + u'': the tile of half 0 waits (E-W summed) in
                             // the other slot, this one is half 1.  First stage across the halves, s = a0 + a1 and
                             // d = (a0 - a1) W_32^{u''} (after the twiddles W_256^{rho u'}), then two FFT-16: s gives the
@@ -809,6 +860,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                             slot_free_arrive(a, sf0 + 8 * s, lane);
                             fft16_detect(a, acc);
                         }
+                        }
                     }
                     // (pointers and the cache policy of the frame end are made here, once per frame: nothing of them is alive
                     // while the tiles are processed, where this role runs at the edge of its registers)
@@ -817,15 +869,36 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                     uint64_t l2_keep;
                     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(l2_keep));
                     const float nrm = prm.norm * __ldg(prm.inv_s2 + c) * kMidDigitUnits2;
-                    // ---- frame end: a9 sum of the two residue halves (+ pol 0), normalise, a10 quantise, 16-byte store per beam
-                    if (res2 == 0) {
+                    // ---- frame end: a9 the fine channels of a beam meet in shared memory (+ pol 0), normalise, a10 quantise,
+                    // 16-byte store per beam.  upchan 128: every thread brings 2 fine channels of the 4 E-W beams of its
+                    // beam, warps 0-3 (E-W beam e2 = rw) take the 16 of (e2, beam).  upchan 256: the even warps bring the 16
+                    // channels of their residue half, the odd ones add theirs.
+                    bool finisher;
+                    if constexpr (U == 128) {
+                        const int g0 = (bitrev(2 * rw, 4) + 8) & 15;     // position 2 rw -> bin bitrev(2 rw); 2 rw + 1 -> 8 further
+                        float *o8 = reinterpret_cast<float *>(smem + kOfsOut) + lane * 17;
 #pragma unroll
-                        for (int g = 0; g < 16; ++g) ost[g] = acc[g];
+                        for (int e = 0; e < 4; ++e) {
+                            o8[e * 32 * 17 + g0] = acc[2 * e];
+                            o8[e * 32 * 17 + (g0 ^ 8)] = acc[2 * e + 1];
+                        }
+                        finisher = rw < 4;
+                    } else {
+                        if (res2 == 0) {
+#pragma unroll
+                            for (int g = 0; g < 16; ++g) ost[g] = acc[g];
+                        }
+                        finisher = res2 == 1;
                     }
                     bar_sync_named(1, 256);
-                    if (res2 == 1) {
+                    if (finisher) {
+                        if constexpr (U == 128) {
 #pragma unroll
-                        for (int g = 0; g < 16; ++g) acc[g] += ost[g];
+                            for (int g = 0; g < 16; ++g) acc[g] = ost[g];
+                        } else {
+#pragma unroll
+                            for (int g = 0; g < 16; ++g) acc[g] += ost[g];
+                        }
                         if (pol == 0) {
 #pragma unroll
                             for (int k = 0; k < 4; ++k)   // parked in L2 (evict_last: 17 MB for the whole grid must survive up to 16 frames of input streaming past)
