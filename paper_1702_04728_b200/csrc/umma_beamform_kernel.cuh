@@ -249,6 +249,121 @@ __device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned cha
     }
 }
 
+// ---- upchan 128: operand preparation by PAIRS of tile types -----------------------------------------------------------
+// Tile types 0 and 1 (residues {0,4}, {2,6}) need the 4-tap butterflies with (-i)^{0 k} and (-i)^{2 k} of the same taps,
+// types 2 and 3 those with (-i)^{k} and (-i)^{3 k}: the first tile of a pair loads the raw rows and splits the nibbles
+// ONCE for both, shares the partial sums of the two butterflies, writes its own B tile and keeps the second tile's
+// (E, O) -- 4 words x 4 values x 2 passes over u' = 32 registers -- for the next call, which then needs no load and no
+// split at all: half the shared-memory reads and a third of the integer instructions of this role.
+// emit_tile: E, O (bytes = value + 32) of one (u', 16-feed chunk) -> the 8 sixteen-byte cells of B tile type TT.
+template <int TT>
+__device__ __forceinline__ void emit_tile(const uint32_t (&er)[4], const uint32_t (&ei)[4], const uint32_t (&orr)[4],
+                                          const uint32_t (&oi)[4], unsigned char *d) {
+    constexpr uint32_t H40 = 0x40404040u, H80 = 0x80808080u;
+    uint32_t re0[4], im0[4], ng0[4], re1[4], im1[4], ng1[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        if constexpr (TT == 0) {          // A_0 = E + O, A_4 = E - O
+            re0[w] = er[w] + orr[w];          im0[w] = ei[w] + oi[w];
+            re1[w] = (er[w] + H40) - orr[w];  im1[w] = (ei[w] + H40) - oi[w];
+            ng0[w] = H80 - re0[w];            ng1[w] = H80 - re1[w];
+        } else if constexpr (TT == 1) {   // A_2 = E + (-i) O, A_6 = E - (-i) O;  (-i)(a + i b) = b - i a
+            re0[w] = er[w] + oi[w];           im0[w] = (ei[w] + H40) - orr[w];
+            re1[w] = (er[w] + H40) - oi[w];   im1[w] = ei[w] + orr[w];
+            ng0[w] = H80 - re0[w];            ng1[w] = H80 - re1[w];
+        } else if constexpr (TT == 2) {   // E_1 (bias 32), O' = (1 - i) O = (a + b) + i (b - a)
+            re0[w] = er[w];                   im0[w] = ei[w];
+            re1[w] = orr[w] + oi[w];          im1[w] = (oi[w] + H40) - orr[w];
+            ng0[w] = H40 - re0[w];            ng1[w] = H80 - re1[w];
+        } else {                          // E_3 (bias 32), O' = (-1 - i) O = (b - a) - i (a + b)
+            re0[w] = er[w];                   im0[w] = ei[w];
+            re1[w] = (oi[w] + H40) - orr[w];  im1[w] = H80 - (orr[w] + oi[w]);
+            ng0[w] = H40 - re0[w];            ng1[w] = H80 - re1[w];
+        }
+    }
+    // biased bytes (value + bias <= 128) -> two's complement bytes: (b + 128 - bias) ^ 0x80, no carry between bytes
+    constexpr uint32_t C0 = (TT < 2) ? 0x40404040u : 0x60606060u, C1 = 0x40404040u;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        re0[w] = (re0[w] + C0) ^ H80;  im0[w] = (im0[w] + C0) ^ H80;  ng0[w] = (ng0[w] + C0) ^ H80;
+        re1[w] = (re1[w] + C1) ^ H80;  im1[w] = (im1[w] + C1) ^ H80;  ng1[w] = (ng1[w] + C1) ^ H80;
+    }
+    *reinterpret_cast<uint4 *>(d) = make_uint4(re0[0], re0[1], re0[2], re0[3]);                 // v0 set0, first half
+    *reinterpret_cast<uint4 *>(d + 1024) = make_uint4(im0[0], im0[1], im0[2], im0[3]);          //          second
+    *reinterpret_cast<uint4 *>(d + 256) = make_uint4(re1[0], re1[1], re1[2], re1[3]);           // v0 set1
+    *reinterpret_cast<uint4 *>(d + 256 + 1024) = make_uint4(im1[0], im1[1], im1[2], im1[3]);
+    *reinterpret_cast<uint4 *>(d + 512) = make_uint4(im0[0], im0[1], im0[2], im0[3]);           // v1 set0
+    *reinterpret_cast<uint4 *>(d + 512 + 1024) = make_uint4(ng0[0], ng0[1], ng0[2], ng0[3]);
+    *reinterpret_cast<uint4 *>(d + 768) = make_uint4(im1[0], im1[1], im1[2], im1[3]);           // v1 set1
+    *reinterpret_cast<uint4 *>(d + 768 + 1024) = make_uint4(ng1[0], ng1[1], ng1[2], ng1[3]);
+}
+
+// The two 4-tap butterflies of a pair from the split nibbles of taps a0 .. a3 (bytes = nibble = value + 8); outputs as
+// int_bfly4's: value + 32 per byte.  PAIR 0: (-i)^{0 k} -> (zr0, zi0), (-i)^{2 k} -> (zr1, zi1); PAIR 1: (-i)^{k}, (-i)^{3 k}.
+template <int PAIR>
+__device__ __forceinline__ void bfly4_pair(const uint32_t (&R)[4], const uint32_t (&I)[4], uint32_t &zr0, uint32_t &zi0,
+                                           uint32_t &zr1, uint32_t &zi1) {
+    constexpr uint32_t B16 = 0x10101010u, B32 = 0x20202020u;
+    if constexpr (PAIR == 0) {
+        const uint32_t ra = R[0] + R[2], rb = R[1] + R[3], ia = I[0] + I[2], ib = I[1] + I[3];
+        zr0 = ra + rb;           zi0 = ia + ib;
+        zr1 = (ra + B32) - rb;   zi1 = (ia + B32) - ib;
+    } else {
+        // x0 - x2 and the cross terms, each + 16 so that no byte goes negative
+        const uint32_t rd = (R[0] + B16) - R[2], id = (I[0] + B16) - I[2], p = (I[1] + B16) - I[3], q = (R[1] + B16) - R[3];
+        zr0 = rd + p;            zi0 = (id + B32) - q;     // (-i)^k:   re = R0 - R2 + I1 - I3, im = I0 - I2 - R1 + R3
+        zr1 = (rd + B32) - p;    zi1 = id + q;             // (-i)^3k:  re = R0 - R2 - I1 + I3, im = I0 - I2 + R1 - R3
+    }
+}
+
+// First tile of a pair (type 2 PAIR): loads, splits, writes tile type 2 PAIR, leaves (E, O) of type 2 PAIR + 1 in keep.
+template <int PAIR>
+__device__ __forceinline__ void prep_pair_first(const unsigned char *raw, unsigned char *bop, const int pw, const int lane,
+                                                uint32_t (&keep)[2][4][4]) {
+    const int j = 4 * pw + (lane >> 3);                 // 16-feed chunk
+    const int x7 = lane & 7;
+    const unsigned char *src = raw + (j >> 3) * (128 * 128) + (((j & 7) ^ x7) << 4);
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const int up = x7 + 8 * it;                     // u'
+        uint4 q[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) q[k] = *reinterpret_cast<const uint4 *>(src + (up + 16 * k) * 128);
+        uint32_t er[4], ei[4], orr[4], oi[4];
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            uint32_t Re[4], Ie[4], Ro[4], Io[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint4 qe = q[2 * k], qo = q[2 * k + 1];
+                split_nibbles(w == 0 ? qe.x : w == 1 ? qe.y : w == 2 ? qe.z : qe.w, Re[k], Ie[k]);
+                split_nibbles(w == 0 ? qo.x : w == 1 ? qo.y : w == 2 ? qo.z : qo.w, Ro[k], Io[k]);
+            }
+            bfly4_pair<PAIR>(Re, Ie, er[w], ei[w], keep[it][w][0], keep[it][w][1]);
+            bfly4_pair<PAIR>(Ro, Io, orr[w], oi[w], keep[it][w][2], keep[it][w][3]);
+        }
+        emit_tile<2 * PAIR>(er, ei, orr, oi, bop + (2 * j) * 1024 + it * 128 + x7 * 16);
+    }
+}
+// Second tile of a pair: from the kept (E, O) only.
+template <int PAIR>
+__device__ __forceinline__ void prep_pair_second(unsigned char *bop, const int pw, const int lane, const uint32_t (&keep)[2][4][4]) {
+    const int j = 4 * pw + (lane >> 3);
+    const int x7 = lane & 7;
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        uint32_t er[4], ei[4], orr[4], oi[4];
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            er[w] = keep[it][w][0];
+            ei[w] = keep[it][w][1];
+            orr[w] = keep[it][w][2];
+            oi[w] = keep[it][w][3];
+        }
+        emit_tile<2 * PAIR + 1>(er, ei, orr, oi, bop + (2 * j) * 1024 + it * 128 + x7 * 16);
+    }
+}
+
 // ---- accumulator drain: one digit pass (64 s32 columns of this thread's lane) folded into 64 partial sums ------------
 // The three digit sums are recombined in INTEGER arithmetic: |a_p| < 2^22 (K 512 x 128 x 64), so u = 256 a2 + a1 fits in
 // 31 bits (one shift-add on the ALU pipe), and v = u + floor(a0 / 256) (one more) is the sum in units of the MIDDLE digit
@@ -548,9 +663,17 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 
     // Register budget per warpgroup: 32 / 80 / 112 / 112 / 72 / 72.  setmaxnreg only redistributes what the CTA was
     // launched with (768 x 80), so the six budgets must not add up to more than 6 x 80.
-    if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
-    else if (warp >= 16) asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
-    else if (warp >= 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+    if constexpr (U == 128) {
+        // upchan 128: 32 / 112 / 112 / 112 / 56 / 56 -- the receive side is one light phase, the preparing warps keep the
+        // second tile of a pair of tile types in registers (the decreases come first: an increase waits for the pool)
+        if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
+        else if (warp >= 16) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        else asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+    } else {
+        if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
+        else if (warp >= 16) asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
+        else if (warp >= 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+    }
 
     if (warp < 2) {
         // ============================== MMA issuers: warp w owns accumulator slot w ==============================
@@ -649,6 +772,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
         // ============================== operand preparation + weight loads ==============================
         const int pw = warp - 4;   // = TMEM lane quarter for the weight loads (warp % 4)
         uint32_t tau = 0, seg = 0, beta = 0;
+        uint32_t keep[2][4][4];    // upchan 128: (E, O) of the second tile of a pair of tile types (prep_pair_first / _second)
         ITEM_LOOP
             for (int pol = 0; pol < 2; ++pol) {
                 if (seg > 0) {
@@ -684,11 +808,20 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 #if defined(CHIME_SKIP) && (CHIME_SKIP & 2)
                             if (prm.n_time < 0)
 #endif
-                            switch (tt) {
-                                case 0: prep_tile<0, U>(raw, bop, pw, lane, h); break;
-                                case 1: prep_tile<1, U>(raw, bop, pw, lane, h); break;
-                                case 2: prep_tile<2, U>(raw, bop, pw, lane, h); break;
-                                default: prep_tile<3, U>(raw, bop, pw, lane, h); break;
+                            if constexpr (U == 128) {
+                                switch (tt) {
+                                    case 0: prep_pair_first<0>(raw, bop, pw, lane, keep); break;
+                                    case 1: prep_pair_second<0>(bop, pw, lane, keep); break;
+                                    case 2: prep_pair_first<1>(raw, bop, pw, lane, keep); break;
+                                    default: prep_pair_second<1>(bop, pw, lane, keep); break;
+                                }
+                            } else {
+                                switch (tt) {
+                                    case 0: prep_tile<0, U>(raw, bop, pw, lane, h); break;
+                                    case 1: prep_tile<1, U>(raw, bop, pw, lane, h); break;
+                                    case 2: prep_tile<2, U>(raw, bop, pw, lane, h); break;
+                                    default: prep_tile<3, U>(raw, bop, pw, lane, h); break;
+                                }
                             }
                             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes -> tensor-core reads
                             asm volatile("bar.arrive %0, %1;" :: "r"(4 + s), "n"(kBopBarThreads) : "memory");   // named barrier: see slot_release
