@@ -2,7 +2,8 @@
 // folded in) runs on the 5th-generation tensor cores as an exact integer GEMM (tcgen05.mma kind::i8), the E-W sum (a5)
 // is an all-to-all over distributed shared memory inside a cluster of 4 CTAs, and the time transform (a7), detection,
 // integration and quantisation (a8-a10) run on the FP32 pipe around it.  Any zero_pad (the padding factor only changes
-// the weights); upchan_len 128 is described below, 256 (template parameter U) where it differs (prep_tile, receive side).  PAPER.md:51-53 (the three kernels), :59-61 (N-S transform), :84-86 (up-channelise).
+// the weights); upchan_len 128 is described below, 256 (template parameter U) where it differs (prep_tile, receive
+// side).  PAPER.md:51-53 (the three kernels), :59-61 (N-S transform), :84-86 (up-channelise).
 //
 // Mathematics.  All operators before |.|^2 are linear and act on different axes, so they commute:
 //   1. time, first stage, on the raw 4-bit integers (exact, packed four feeds per register): with t = u' + 16 k,
@@ -19,9 +20,11 @@
 //      (drain_pass).  Real and imaginary outputs of a beam come
 //      from the SAME weight row [Wr | -Wi] applied to two variants of the data column, [re | im] and [im | -re], so
 //      both land in the same TMEM lane (= thread) in different columns.
-//   3. E-W: Z_e = sum_cyl beta_e^cyl S_cyl (Horner), after an all-to-all by beam quarter over DSMEM: CTA r of the
-//      cluster owns cylinder r on the way in and beams 32 r .. 32 r + 31 of the tile on the way out.
-//   4. time, second stage, per (beam, residue, E-W beam): twiddle W_128^{rho u'}, FFT-16 over u'.
+//   3. time, second stage, per (beam, residue, cylinder): twiddle W_128^{rho u'}, FFT-16 over u' -- in the drain, on the
+//      values of a beam that are in registers there (upchan 128; upchan 256 needs both halves of u' and runs this
+//      stage after the E-W sum, on the receiving side).
+//   4. E-W: Z_e = sum_cyl beta_e^cyl S_cyl (Horner) per frequency bin, after an all-to-all by beam quarter over DSMEM:
+//      CTA r of the cluster owns cylinder r on the way in and beams 32 r .. 32 r + 31 of the tile on the way out.
 //   5. |Z|^2, sum over the 8 bins of a fine channel (= over rho), the 2 polarisations and the 3 blocks; quantise.
 //
 // Work decomposition: item = (channel, tile of 128 beams, chunk of up to 16 output frames), handed round-robin to the
@@ -33,10 +36,12 @@
 //
 // Warp roles (768 threads, 1 CTA / SM):
 //   warps 0-1     MMA issuers (warp w owns accumulator slot w)   warps 2-3   raw-block staging (one lane, TMA)
-//   warps 4-7     operand preparation (integer butterflies -> K-major B tile), weight loads into TMEM
-//   warps 8-15    accumulator drain (tcgen05.ld), digit recombination, E +- O'/sqrt2, DSMEM send;
+//   warps 4-7     operand preparation (integer butterflies -> K-major B tile; by pairs of tile types that share the
+//                 taps), weight loads into TMEM
+//   warps 8-15    accumulator drain (tcgen05.ld), digit recombination, E +- O'/sqrt2, twiddle + FFT-16, DSMEM send;
 //                 warps 8-11 take even tiles, 12-15 odd tiles; warp % 4 = TMEM lane quarter = destination CTA
-//   warps 16-23   receive side: E-W Horner, twiddle, FFT-16, detect, accumulate; frame end (normalise, quantise, store)
+//   warps 16-23   receive side: E-W Horner per frequency bin, detect, accumulate (one phase, no barrier per tile);
+//                 frame end (fine channels gathered in shared memory, normalise, quantise, store)
 // Hand-overs: mbarriers where an asynchronous unit or another CTA signals (TMA, tcgen05.commit, st.async, remote
 // arrive), named barriers for the two latency-critical local ones (slot drained, B tile written).
 #pragma once
@@ -56,7 +61,8 @@ using chime::fft_dif;
 constexpr int kThreads = 768;
 constexpr int kMaxChunkFrames = 16;             // most output frames per item (polarisation-0 sums wait in the scratch)
 constexpr int kRawBytes = 128 * 256;            // one (block, pol, cylinder): 32 KiB
-constexpr int kBopBytes = 64 * 512;             // one B tile: 64 columns x K 512 bytes
+constexpr int kBopKStep = 3 * 512;              // one K step (32 bytes of K) of a B tile: [re | im | -re] chunks of 32 rows x 16 bytes
+constexpr int kBopBytes = 16 * kBopKStep;       // one B tile: 24 KiB for 64 columns x K 512 (the two variants share the im chunk)
 constexpr int kRecvBytes = 4 * 2 * 8 * 32 * 16; // one receive slot: [cyl][res][i pair][beam][2 x float2] = 32 KiB
 constexpr int kOfsRaw = 0, kOfsBop = 2 * kRawBytes, kOfsRecv = kOfsBop + 2 * kBopBytes;
 constexpr int kOfsOut = kOfsRecv + 2 * kRecvBytes;
@@ -185,7 +191,11 @@ __device__ __forceinline__ void bar_sync_named(int id, int n) { asm volatile("ba
 // TT = 0: columns A_0, A_4; 1: A_2, A_6; 2: E_1, O'_1; 3: E_3, O'_3.  B tile row n = 32 variant + 16 set + u',
 // K byte 32 j + i (i < 16): first half of feed 16 j + i, 32 j + 16 + i: second half; variant 0 = [re | im],
 // variant 1 = [im | -re]; signed bytes (the packed butterflies run on biased bytes, bias 64 (A, O') or 32 (E), which is
-// removed at the end).  Layout [kc = K/16][row group 8][8 rows][16 B].
+// removed at the end).  Layout per K step j (32 bytes of K): three chunks of [32 rows of variant 0][16 B] -- re, im, -re;
+// the descriptor's K-adjacent core matrix is 512 bytes on (LBO) and its row groups 128 bytes apart (SBO), so that row
+// group 4 + g of K chunk 0 IS row group g of K chunk 1: variant 1's [im | -re] reads the im chunk that variant 0 reads
+// as its second half and the -re chunk behind it.  24 KiB per tile instead of 32, 6 stores per thread and pass over u'
+// instead of 8.
 // U = 256: a block is 256 samples, t = u' + 32 k with u' = 16 h + (0 .. 15): the tile takes the 16 values of u' of half
 // h, the block sits in shared memory as [feed half][256 rows][128 B] (64 KiB, both raw buffers).
 template <int TT, int U>
@@ -237,15 +247,13 @@ __device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned cha
             re1[w] = (re1[w] + C1) ^ H80;  im1[w] = (im1[w] + C1) ^ H80;  ng1[w] = (ng1[w] + C1) ^ H80;
         }
         // rows: variant 0 set s: 16 s + u';  variant 1: 32 + 16 s + u'.  (row >> 3) * 128 + (row & 7) * 16
-        unsigned char *d = bop + (2 * j) * 1024 + it * 128 + x7 * 16;
-        *reinterpret_cast<uint4 *>(d) = make_uint4(re0[0], re0[1], re0[2], re0[3]);                 // v0 set0, first half
-        *reinterpret_cast<uint4 *>(d + 1024) = make_uint4(im0[0], im0[1], im0[2], im0[3]);          //          second
-        *reinterpret_cast<uint4 *>(d + 256) = make_uint4(re1[0], re1[1], re1[2], re1[3]);           // v0 set1
-        *reinterpret_cast<uint4 *>(d + 256 + 1024) = make_uint4(im1[0], im1[1], im1[2], im1[3]);
-        *reinterpret_cast<uint4 *>(d + 512) = make_uint4(im0[0], im0[1], im0[2], im0[3]);           // v1 set0
-        *reinterpret_cast<uint4 *>(d + 512 + 1024) = make_uint4(ng0[0], ng0[1], ng0[2], ng0[3]);
-        *reinterpret_cast<uint4 *>(d + 768) = make_uint4(im1[0], im1[1], im1[2], im1[3]);           // v1 set1
-        *reinterpret_cast<uint4 *>(d + 768 + 1024) = make_uint4(ng1[0], ng1[1], ng1[2], ng1[3]);
+        unsigned char *d = bop + j * kBopKStep + it * 128 + x7 * 16;
+        *reinterpret_cast<uint4 *>(d) = make_uint4(re0[0], re0[1], re0[2], re0[3]);                 // re chunk: set 0
+        *reinterpret_cast<uint4 *>(d + 256) = make_uint4(re1[0], re1[1], re1[2], re1[3]);           //           set 1
+        *reinterpret_cast<uint4 *>(d + 512) = make_uint4(im0[0], im0[1], im0[2], im0[3]);           // im chunk
+        *reinterpret_cast<uint4 *>(d + 768) = make_uint4(im1[0], im1[1], im1[2], im1[3]);
+        *reinterpret_cast<uint4 *>(d + 1024) = make_uint4(ng0[0], ng0[1], ng0[2], ng0[3]);          // -re chunk
+        *reinterpret_cast<uint4 *>(d + 1280) = make_uint4(ng1[0], ng1[1], ng1[2], ng1[3]);
     }
 }
 
@@ -288,14 +296,12 @@ __device__ __forceinline__ void emit_tile(const uint32_t (&er)[4], const uint32_
         re0[w] = (re0[w] + C0) ^ H80;  im0[w] = (im0[w] + C0) ^ H80;  ng0[w] = (ng0[w] + C0) ^ H80;
         re1[w] = (re1[w] + C1) ^ H80;  im1[w] = (im1[w] + C1) ^ H80;  ng1[w] = (ng1[w] + C1) ^ H80;
     }
-    *reinterpret_cast<uint4 *>(d) = make_uint4(re0[0], re0[1], re0[2], re0[3]);                 // v0 set0, first half
-    *reinterpret_cast<uint4 *>(d + 1024) = make_uint4(im0[0], im0[1], im0[2], im0[3]);          //          second
-    *reinterpret_cast<uint4 *>(d + 256) = make_uint4(re1[0], re1[1], re1[2], re1[3]);           // v0 set1
-    *reinterpret_cast<uint4 *>(d + 256 + 1024) = make_uint4(im1[0], im1[1], im1[2], im1[3]);
-    *reinterpret_cast<uint4 *>(d + 512) = make_uint4(im0[0], im0[1], im0[2], im0[3]);           // v1 set0
-    *reinterpret_cast<uint4 *>(d + 512 + 1024) = make_uint4(ng0[0], ng0[1], ng0[2], ng0[3]);
-    *reinterpret_cast<uint4 *>(d + 768) = make_uint4(im1[0], im1[1], im1[2], im1[3]);           // v1 set1
-    *reinterpret_cast<uint4 *>(d + 768 + 1024) = make_uint4(ng1[0], ng1[1], ng1[2], ng1[3]);
+    *reinterpret_cast<uint4 *>(d) = make_uint4(re0[0], re0[1], re0[2], re0[3]);                 // re chunk: set 0
+    *reinterpret_cast<uint4 *>(d + 256) = make_uint4(re1[0], re1[1], re1[2], re1[3]);           //           set 1
+    *reinterpret_cast<uint4 *>(d + 512) = make_uint4(im0[0], im0[1], im0[2], im0[3]);           // im chunk
+    *reinterpret_cast<uint4 *>(d + 768) = make_uint4(im1[0], im1[1], im1[2], im1[3]);
+    *reinterpret_cast<uint4 *>(d + 1024) = make_uint4(ng0[0], ng0[1], ng0[2], ng0[3]);          // -re chunk
+    *reinterpret_cast<uint4 *>(d + 1280) = make_uint4(ng1[0], ng1[1], ng1[2], ng1[3]);
 }
 
 // The two 4-tap butterflies of a pair from the split nibbles of taps a0 .. a3 (bytes = nibble = value + 8); outputs as
@@ -342,7 +348,7 @@ __device__ __forceinline__ void prep_pair_first(const unsigned char *raw, unsign
             bfly4_pair<PAIR>(Re, Ie, er[w], ei[w], keep[it][w][0], keep[it][w][1]);
             bfly4_pair<PAIR>(Ro, Io, orr[w], oi[w], keep[it][w][2], keep[it][w][3]);
         }
-        emit_tile<2 * PAIR>(er, ei, orr, oi, bop + (2 * j) * 1024 + it * 128 + x7 * 16);
+        emit_tile<2 * PAIR>(er, ei, orr, oi, bop + j * kBopKStep + it * 128 + x7 * 16);
     }
 }
 // Second tile of a pair: from the kept (E, O) only.
@@ -360,7 +366,7 @@ __device__ __forceinline__ void prep_pair_second(unsigned char *bop, const int p
             orr[w] = keep[it][w][2];
             oi[w] = keep[it][w][3];
         }
-        emit_tile<2 * PAIR + 1>(er, ei, orr, oi, bop + (2 * j) * 1024 + it * 128 + x7 * 16);
+        emit_tile<2 * PAIR + 1>(er, ei, orr, oi, bop + j * kBopKStep + it * 128 + x7 * 16);
     }
 }
 
@@ -694,7 +700,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                     const uint32_t s = tau & 1, ph = (tau >> 1) & 1;
                     (void)ph;
                     PW(2, asm volatile("bar.sync %0, %1;" :: "r"(4 + s), "n"(kBopBarThreads) : "memory");)   // the B tile is written
-                    const uint64_t bd0 = make_desc(smem_u32(smem + kOfsBop) + s * kBopBytes, 1024, 128);
+                    const uint64_t bd0 = make_desc(smem_u32(smem + kOfsBop) + s * kBopBytes, 512, 128);
 #pragma unroll 1
                     for (uint32_t p = 0; p < 3; ++p) {
                         const uint32_t pi = 3 * tau + p;
@@ -724,7 +730,7 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll 1
                             for (int k = 1; k < 16; ++k) {   // rolled: the issuers run on 32 registers
                                 a += 8;
-                                bd += 2048 >> 4;
+                                bd += kBopKStep >> 4;
                                 umma_i8_ts<true>(d, a, bd, idesc);
                             }
                             umma_commit(BAR(B_ACC_FULL + 2 * g + myslot));
