@@ -544,6 +544,22 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const 
                 y[32 * set + 2 * u + 1] = __float_as_uint(a[u].y);
             }
         }
+    } else {
+        // upchan 256: the twiddles W_256^{rho u'}, u' = 16 h + u'', are applied here too (the same factor for the four
+        // cylinders of a beam, so before the E-W sum as well as after it); the 32-point transform itself needs both
+        // halves h, which are two tiles and two drain groups: it stays on the receiving side.
+        const int h = tau & 1;
+#pragma unroll
+        for (int set = 0; set < 2; ++set) {
+            const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * set;
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                const float2 v = chime::cmul(make_float2(__uint_as_float(y[32 * set + 2 * u]), __uint_as_float(y[32 * set + 2 * u + 1])),
+                                             c_twr256[rho][16 * h + u]);
+                y[32 * set + 2 * u] = __float_as_uint(v.x);
+                y[32 * set + 2 * u + 1] = __float_as_uint(v.y);
+            }
+        }
     }
     const uint32_t rslot = mapa(recv0 + g * kRecvBytes, q), rbar = mapa(bar0 + 8u * (B_RECV_FULL + g), q);
     PW(5, mbar_wait(bar0 + 8u * (B_SLOT_FREE + 2 * q + g), ((tau >> 1) & 1) ^ 1, prm, 5);)     // the destination has consumed this slot's previous tile
@@ -950,13 +966,11 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                         if (t & 1) {
                             // U = 256: the FFT over u' has 32 points, u' = 16 h + u'': the tile of half 0 waits (E-W summed) in
                             // the other slot, this one is half 1.  First stage across the halves, s = a0 + a1 and
-                            // d = (a0 - a1) W_32^{u''} (after the twiddles W_256^{rho u'}), then two FFT-16: s gives the
+                            // d = (a0 - a1) W_32^{u''} (the twiddles W_256^{rho u'} were applied by the senders), then two FFT-16: s gives the
                             // even bins, d the odd ones.  d waits in this thread's own cells of the slot meanwhile.
                             bar_sync_named(1, 256);   // (covers phase 1 of the previous tile too: no barrier on even tiles)
                             unsigned char *base1 = slot + ((e2 * 2 + res2) * 8) * 512;
                             unsigned char *base0 = base1 + (s ? -kRecvBytes : kRecvBytes);
-                            const int tt = (t >> 1) & 3;
-                            const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * res2;
 #pragma unroll
                             for (int k = 0; k < 8; ++k) {
                                 const float4 v0 = *reinterpret_cast<const float4 *>(base0 + k * 512);
@@ -967,8 +981,6 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                                     const int u = 2 * k + j;
                                     float2 p0 = j ? make_float2(v0.z, v0.w) : make_float2(v0.x, v0.y);
                                     float2 p1 = j ? make_float2(v1.z, v1.w) : make_float2(v1.x, v1.y);
-                                    if (u > 0) p0 = chime::cmul(p0, c_twr256[rho][u]);
-                                    p1 = chime::cmul(p1, c_twr256[rho][16 + u]);
                                     sm[j] = chime::cadd(p0, p1);
                                     d[j] = chime::csub(p0, p1);
                                     if (u > 0) d[j] = chime::cmul(d[j], c_w32[u]);
