@@ -20,9 +20,10 @@
 //      (drain_pass).  Real and imaginary outputs of a beam come
 //      from the SAME weight row [Wr | -Wi] applied to two variants of the data column, [re | im] and [im | -re], so
 //      both land in the same TMEM lane (= thread) in different columns.
-//   3. time, second stage, per (beam, residue, cylinder): twiddle W_128^{rho u'}, FFT-16 over u' -- in the drain, on the
-//      values of a beam that are in registers there (upchan 128; upchan 256 needs both halves of u' and runs this
-//      stage after the E-W sum, on the receiving side).
+//   3. time, second stage, per (beam, residue, cylinder): twiddle W_U^{rho u'}, FFT-16 -- in the drain, on the values of
+//      a beam that are in registers there.  upchan 128: over u' = 0 .. 15, the whole stage.  upchan 256: u' = 2 u'' + h, a
+//      tile holds the even (h = 0) or odd (h = 1) u' and its FFT-16 over u'' is one branch of a decimation-in-time
+//      FFT-32; the last butterfly, across the two tiles of a residue pair, follows the E-W sum on the receiving side.
 //   4. E-W: Z_e = sum_cyl beta_e^cyl S_cyl (Horner) per frequency bin, after an all-to-all by beam quarter over DSMEM:
 //      CTA r of the cluster owns cylinder r on the way in and beams 32 r .. 32 r + 31 of the tile on the way out.
 //   5. |Z|^2, sum over the 8 bins of a fine channel (= over rho), the 2 polarisations and the 3 blocks; quantise.
@@ -40,8 +41,9 @@
 //                 taps), weight loads into TMEM
 //   warps 8-15    accumulator drain (tcgen05.ld), digit recombination, E +- O'/sqrt2, twiddle + FFT-16, DSMEM send;
 //                 warps 8-11 take even tiles, 12-15 odd tiles; warp % 4 = TMEM lane quarter = destination CTA
-//   warps 16-23   receive side: E-W Horner per frequency bin, detect, accumulate (one phase, no barrier per tile);
-//                 frame end (fine channels gathered in shared memory, normalise, quantise, store)
+//   warps 16-23   receive side: E-W Horner per frequency bin (upchan 256: + the last butterfly of the FFT-32 across two
+//                 tiles), detect, accumulate (one phase, no barrier per tile); frame end (fine channels gathered in
+//                 shared memory, normalise, quantise, store)
 // Hand-overs: mbarriers where an asynchronous unit or another CTA signals (TMA, tcgen05.commit, st.async, remote
 // arrive), named barriers for the two latency-critical local ones (slot drained, B tile written).
 #pragma once
@@ -66,7 +68,7 @@ constexpr int kBopBytes = 16 * kBopKStep;       // one B tile: 24 KiB for 64 col
 constexpr int kRecvBytes = 4 * 2 * 8 * 32 * 16; // one receive slot: [cyl][res][i pair][beam][2 x float2] = 32 KiB
 constexpr int kOfsRaw = 0, kOfsBop = 2 * kRawBytes, kOfsRecv = kOfsBop + 2 * kBopBytes;
 constexpr int kOfsOut = kOfsRecv + 2 * kRecvBytes;
-constexpr int kOutBytes = 4 * 32 * 17 * 4;      // [e][beam][16 + 1 pad] floats
+constexpr int kOutBytes = 2 * 4 * 32 * 17 * 4;  // [half][e][beam][16 + 1 pad] floats (the second half: upchan 256 only)
 constexpr int kOfsBar = kOfsOut + kOutBytes;
 // mbarrier indices
 enum { B_RAW_FULL = 0, B_RAW_EMPTY = 2, B_BOP_EMPTY = 6, B_RECV_FULL = 12, B_SLOT_FREE = 14 /* [dest 4][slot 2] */,
@@ -196,8 +198,8 @@ __device__ __forceinline__ void bar_sync_named(int id, int n) { asm volatile("ba
 // group 4 + g of K chunk 0 IS row group g of K chunk 1: variant 1's [im | -re] reads the im chunk that variant 0 reads
 // as its second half and the -re chunk behind it.  24 KiB per tile instead of 32, 6 stores per thread and pass over u'
 // instead of 8.
-// U = 256: a block is 256 samples, t = u' + 32 k with u' = 16 h + (0 .. 15): the tile takes the 16 values of u' of half
-// h, the block sits in shared memory as [feed half][256 rows][128 B] (64 KiB, both raw buffers).
+// U = 256: a block is 256 samples, t = u' + 32 k with u' = 2 u'' + h: the tile takes the 16 even (h = 0) or odd (h = 1)
+// values of u', the block sits in shared memory as [feed half][256 rows][128 B] (64 KiB, both raw buffers).
 template <int TT, int U>
 __device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned char *bop, const int pw, const int lane, const int h) {
     constexpr int R4 = (TT == 0) ? 0 : (TT == 1) ? 2 : (TT == 2) ? 1 : 3;
@@ -205,13 +207,17 @@ __device__ __forceinline__ void prep_tile(const unsigned char *raw, unsigned cha
     const int j = 4 * pw + (lane >> 3);                 // 16-feed chunk
     const int x7 = lane & 7;
     constexpr int kTap = U / 8;                         // row distance of the 8 taps of a residue
-    const unsigned char *src = raw + (j >> 3) * (U * 128) + (((j & 7) ^ x7) << 4) + (U == 256 ? h * 2048 : 0);
+    // U = 128: tap k of u' is row u' + 16 k.  U = 256: the tile of half h takes u' = 2 u'' + h (the even or the odd u' of
+    // the 32: the two FFT-16 over u'' of a decimation-in-time FFT-32), tap k is row 2 u'' + h + 32 k; the 128-byte swizzle
+    // of the staged block follows the row (row & 7 = (2 u'' + h) & 7).
+    const unsigned char *src = U == 128 ? raw + (j >> 3) * (U * 128) + (((j & 7) ^ x7) << 4)
+                                        : raw + (j >> 3) * (U * 128) + (((j & 7) ^ ((2 * x7 + h) & 7)) << 4) + h * 128;
 #pragma unroll 1
     for (int it = 0; it < 2; ++it) {
         const int up = x7 + 8 * it;                     // u'
         uint4 q[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) q[k] = *reinterpret_cast<const uint4 *>(src + (up + kTap * k) * 128);
+        for (int k = 0; k < 8; ++k) q[k] = *reinterpret_cast<const uint4 *>(src + ((U == 128 ? up : 2 * up) + kTap * k) * 128);
         uint32_t re0[4], im0[4], ng0[4], re1[4], im1[4], ng1[4];
 #pragma unroll
         for (int w = 0; w < 4; ++w) {
@@ -484,7 +490,7 @@ __device__ __forceinline__ void drain_pass(const uint32_t tslot, uint32_t (&y)[6
 // Group g takes the tiles tau = 2 k + g: its passes use slots g, g ^ 1, g, so tile k is uses 2 k, 2 k + 1 of barrier
 // ACC_FULL[g][g] and use k of ACC_FULL[g][g ^ 1]: the parities are 0, k & 1, 1 -- no counters.  Everything that is only
 // needed after the three passes (destination addresses) is computed there: the drain runs at the edge of its registers.
-template <bool DRAIN_FFT>
+template <int U>
 __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const uint32_t bar0, const uint32_t recv0, const uint32_t g,
                                          const uint32_t q, const uint32_t tau, const int cyl, const int lane, const Params &prm,
                                          long long *prof_w) {
@@ -522,42 +528,34 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const 
             y[32 + k] = __float_as_uint(fmaf(-s, o, e));
         }
     }
-    if constexpr (DRAIN_FFT) {
-        // upchan 128: the rest of the time transform (twiddle W_128^{rho u'}, FFT-16 over u') runs HERE, on the 2 x 16
-        // values of this thread's beam that are in registers anyway, before the E-W sum instead of after it (both are
-        // linear and act on different axes).  The receive side is then one phase -- E-W sum per frequency bin, |.|^2 --
-        // with no write-back, no re-read and no barrier per tile: a third of its shared-memory traffic, on the pipe
-        // that the tensor core's operand reads share.  Position i of a set afterwards holds bin
-        // bitrev(i) of the 16-point transform.
+    {
+        // The rest of the time transform runs HERE, on the 2 x 16 values of this thread's beam that are in registers
+        // anyway, before the E-W sum instead of after it (both are linear and act on different axes): twiddle
+        // W_U^{rho u'} and FFT-16.  upchan 128: u' = 0 .. 15, that is the whole second stage.  upchan 256: u' = 2 u'' + h,
+        // the FFT-16 over u'' is the half-h branch of a decimation-in-time FFT-32 whose last butterfly (across the two
+        // tiles h = 0, 1 of a residue pair) is left to the receive side.  The receive side is then one phase -- E-W sum per
+        // frequency bin, |.|^2 -- with no write-back, no re-read and no barrier per tile: a third of its shared-memory
+        // traffic, on the pipe that the tensor core's operand reads share.  Position i of a set
+        // afterwards holds bin bitrev(i) of the 16-point transform.
+        const int h = tau & 1;      // (upchan 256: tiles come as (residue pair, h) with h fastest)
 #pragma unroll
         for (int set = 0; set < 2; ++set) {
             const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * set;      // residues {0,4}, {2,6}, {1,5}, {3,7} by tile type
             float2 a[16];
 #pragma unroll
             for (int u = 0; u < 16; ++u) a[u] = make_float2(__uint_as_float(y[32 * set + 2 * u]), __uint_as_float(y[32 * set + 2 * u + 1]));
+            if constexpr (U == 128) {
 #pragma unroll
-            for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr[rho][u]);
+                for (int u = 1; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr[rho][u]);
+            } else {
+#pragma unroll
+                for (int u = 0; u < 16; ++u) a[u] = chime::cmul(a[u], c_twr256[rho][2 * u + h]);
+            }
             fft_dif<16>(a);
 #pragma unroll
             for (int u = 0; u < 16; ++u) {
                 y[32 * set + 2 * u] = __float_as_uint(a[u].x);
                 y[32 * set + 2 * u + 1] = __float_as_uint(a[u].y);
-            }
-        }
-    } else {
-        // upchan 256: the twiddles W_256^{rho u'}, u' = 16 h + u'', are applied here too (the same factor for the four
-        // cylinders of a beam, so before the E-W sum as well as after it); the 32-point transform itself needs both
-        // halves h, which are two tiles and two drain groups: it stays on the receiving side.
-        const int h = tau & 1;
-#pragma unroll
-        for (int set = 0; set < 2; ++set) {
-            const int rho = ((tt & 1) << 1) + (tt >> 1) + 4 * set;
-#pragma unroll
-            for (int u = 0; u < 16; ++u) {
-                const float2 v = chime::cmul(make_float2(__uint_as_float(y[32 * set + 2 * u]), __uint_as_float(y[32 * set + 2 * u + 1])),
-                                             c_twr256[rho][16 * h + u]);
-                y[32 * set + 2 * u] = __float_as_uint(v.x);
-                y[32 * set + 2 * u + 1] = __float_as_uint(v.y);
             }
         }
     }
@@ -576,27 +574,10 @@ __device__ __forceinline__ void epi_tile(const int tt, const uint32_t tb, const 
         }
 }
 
-// Receive side, helpers of phase 2.  slot_free_arrive: "this warp has its part of receive slot s in registers" to the
-// four sending CTAs.  The arrive is made to depend on one word of every load (a[1], a[3], ... come from the 8 loads),
-// so that it cannot be issued while a load is still in flight.
-// sf_local = this CTA's own SLOT_FREE barrier of (its beams, slot s): the same offset in each source CTA (mapa at the
-// point of use: four live registers less on a role that runs at the edge of its 72).
-__device__ __forceinline__ void slot_free_arrive(const float2 (&a)[16], const uint32_t sf_local, const int lane) {
-    uint32_t dep;
-    asm volatile("{ .reg .b32 t0, t1;\n or.b32 t0, %1, %2;\n or.b32 t1, %3, %4;\n or.b32 t0, t0, t1;\n"
-                 " or.b32 t1, %5, %6;\n or.b32 t0, t0, t1;\n or.b32 t1, %7, %8;\n or.b32 t0, t0, t1;\n"
-                 " or.b32 %0, t0, 1; }"
-                 : "=r"(dep)
-                 : "r"(__float_as_uint(a[1].y)), "r"(__float_as_uint(a[3].y)), "r"(__float_as_uint(a[5].y)),
-                   "r"(__float_as_uint(a[7].y)), "r"(__float_as_uint(a[9].y)), "r"(__float_as_uint(a[11].y)),
-                   "r"(__float_as_uint(a[13].y)), "r"(__float_as_uint(a[15].y)));
-    dep = __reduce_or_sync(0xffffffffu, dep);   // every lane's loads
-    if (lane == 0 && dep != 0) {
-#pragma unroll
-        for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(mapa(sf_local, sc));
-    }
-}
-// (upchan 128: the 8 sixteen-byte loads of the single receive phase)
+// Receive side: "this warp has its part of receive slot s in registers" to the four sending CTAs.  The arrive is made
+// to depend on one word of every one of the 8 sixteen-byte loads, so that it cannot be issued while a load is still in
+// flight.  sf_local = this CTA's own SLOT_FREE barrier of (its beams, slot s): the same offset in each source CTA (mapa
+// at the point of use).
 __device__ __forceinline__ void slot_free_arrive(const float4 (&v)[2][4], const uint32_t sf_local, const int lane) {
     uint32_t dep;
     asm volatile("{ .reg .b32 t0, t1;\n or.b32 t0, %1, %2;\n or.b32 t1, %3, %4;\n or.b32 t0, t0, t1;\n"
@@ -612,18 +593,6 @@ __device__ __forceinline__ void slot_free_arrive(const float4 (&v)[2][4], const 
         for (int sc = 0; sc < 4; ++sc) mbar_arrive_remote_relaxed(mapa(sf_local, sc));
     }
 }
-// FFT-16 over u' (input already twiddled), |.|^2 into the 16 fine channels: output bin q of the transform belongs to
-// fine channel (q + 8) & 15 for both up-channelisation lengths (U = 128: bin 8 q + rho of 128, 8 bins per fine channel;
-// U = 256: bins 8 (2 q) + rho and 8 (2 q + 1) + rho of 256, 16 per fine channel).
-__device__ __forceinline__ void fft16_detect(float2 (&a)[16], float (&acc)[16]) {
-    fft_dif<16>(a);
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const int g = (bitrev(i, 4) + 8) & 15;
-        acc[g] = fmaf(a[i].x, a[i].x, fmaf(a[i].y, a[i].y, acc[g]));
-    }
-}
-
 // tmap: the packed baseband as a 2-D byte tensor [C * T rows][2048], box 128 bytes x 128 rows, 128-byte swizzle (the
 // layout prep_tile reads: 16-byte chunk index ^ (row & 7) inside every 128-byte row).
 // U = upchan_len (128 or 256): a frame is 3 blocks of U samples = 3 U / 32 tiles per polarisation.
@@ -864,21 +833,20 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll 1
                 for (int t = ntiles; t > 0; --t, ++tau) {   // (tiles per frame and polarisation: a multiple of 8, so tau gives the tile type)
                     if ((tau & 1) != g) continue;
-                    epi_tile<U == 128>(U == 128 ? (tau & 3) : ((tau >> 1) & 3), tb, bar0, recv0, g, q, tau, rank, lane, prm, prof_w);
+                    epi_tile<U>(U == 128 ? (tau & 3) : ((tau >> 1) & 3), tb, bar0, recv0, g, q, tau, rank, lane, prm, prof_w);
                 }
             }
         }
     } else {
         // ============================== receive side: E-W, time FFT-16, detect, integrate, output ==============================
-        // Two phases per tile over the slot [cyl][res][u' pair][beam] x {re, im, re, im}:
-        //   1. thread <-> (beam = lane, u' pair = warp): Horner in beta_e over the 4 cylinders for both residues, the 4
-        //      E-W beams written back IN PLACE (cell index cyl -> e);
-        //   2. thread <-> (beam, residue = warp & 1, E-W beam = warp >> 1): 16 values of u', twiddle W_128^{rho u'},
-        //      FFT-16, |.|^2 into the 16 fine channels of the current frame.
-        // Per frame the two residue halves meet in shared memory and the odd warps, which then hold all 16 fine channels
+        // One phase over the slot [cyl][res][position pair][beam] x {re, im, re, im}, whose positions hold frequency bins
+        // (the senders ran the FFT-16): thread <-> (beam = lane, position pair = warp) sums the 4 cylinders into the 4 E-W
+        // beams (Horner in beta_e) for both residues and detects -- per tile at upchan 128, per pair of tiles (the two
+        // halves of a decimation-in-time FFT-32, with its last butterfly) at upchan 256.  No store, no barrier per tile.
+        // Per frame the fine channels of a beam meet in shared memory and warps 16-19, which then hold all 16 fine channels
         // of (E-W beam, beam), park the polarisation-0 sums in a per-CTA scratch (L2) and finish the frame after pol 1.
         const int rw = warp - 16;
-        const int res2 = rw & 1, e2 = U == 128 ? (rw & 3) : (rw >> 1);   // upchan 128: e2 = E-W beam of the frame-end role (warps 0-3)
+        const int e2 = rw & 3;   // E-W beam of the frame-end role (warps 16-19)
         const uint32_t sf0 = BAR(B_SLOT_FREE + 2 * rank);   // slot 0's barrier of this CTA's beams (in every source CTA); slot 1's is 8 bytes further
         uint32_t tau = 0;
         ITEM_LOOP
@@ -932,21 +900,59 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                                     acc[2 * e] = fmaf(za.x, za.x, fmaf(za.y, za.y, acc[2 * e]));
                                     acc[2 * e + 1] = fmaf(zb.x, zb.x, fmaf(zb.y, zb.y, acc[2 * e + 1]));
                                 }
-                        } else {
-#if defined(CHIME_SKIP) && (CHIME_SKIP & 16)
-                        if (prm.n_time < 0)
-#endif
-                        {   // ---- phase 1: (beam, u' pair = rw), both residues
-                            unsigned char *base = slot + rw * 512;
+                        } else if (t & 1) {
+                            // ---- upchan 256: ONE phase per PAIR of tiles.  The tile of half 0 (even u', bins E of a decimation-in-
+                            // time FFT-32) waits in the other slot, this one is half 1 (odd u', bins O); the senders have run the
+                            // FFT-16 over u''.  Thread <-> (beam = lane, position pair = rw): E-W sum of both halves, the last
+                            // butterfly X[q] = E[q] + W_32^q O[q], X[q + 16] = E[q] - W_32^q O[q] for the positions' bins q = qa, qa + 8,
+                            // |.|^2 into 4 x 4 partial intensities (fine channels (qa >> 1) + 8, qa >> 1, + 12, + 4).
+                            const unsigned char *b1 = slot + rw * 512;
+                            const unsigned char *b0 = b1 + (s ? -kRecvBytes : kRecvBytes);
+                            const int qa = bitrev(rw, 3);
+                            const float2 wa = c_w32[qa], wb = c_w32[qa + 8];
+                            uint32_t dep = 0;
 #pragma unroll
                             for (int res = 0; res < 2; ++res) {
+                                float2 z0a[4], z0b[4];      // E-W sums of half 0, positions 2 rw and 2 rw + 1
+                                {
+                                    float4 sv[4];
+#pragma unroll
+                                    for (int cy = 0; cy < 4; ++cy)
+                                        sv[cy] = *reinterpret_cast<const float4 *>(b0 + ((cy * 2 + res) * 8) * 512);
+                                    dep |= __float_as_uint(sv[0].w) | __float_as_uint(sv[1].w) | __float_as_uint(sv[2].w) | __float_as_uint(sv[3].w);
+#pragma unroll
+                                    for (int e = 0; e < 4; ++e) {
+                                        const float2 bx = make_float2(be[e].x, be[e].x), by = make_float2(-be[e].y, be[e].y);
+                                        float2 za = make_float2(sv[3].x, sv[3].y), zb = make_float2(sv[3].z, sv[3].w);
+#pragma unroll
+                                        for (int cy = 2; cy >= 0; --cy) {
+                                            const float2 sa = make_float2(sv[cy].x, sv[cy].y), sb = make_float2(sv[cy].z, sv[cy].w);
+                                            const float2 ta = __ffma2_rn(za, bx, sa), tb2 = __ffma2_rn(zb, bx, sb);
+                                            za = __ffma2_rn(make_float2(za.y, za.x), by, ta);
+                                            zb = __ffma2_rn(make_float2(zb.y, zb.x), by, tb2);
+                                        }
+                                        z0a[e] = za;
+                                        z0b[e] = zb;
+                                    }
+                                }
                                 float4 sv[4];
 #pragma unroll
                                 for (int cy = 0; cy < 4; ++cy)
-                                    sv[cy] = *reinterpret_cast<const float4 *>(base + ((cy * 2 + res) * 8) * 512);
+                                    sv[cy] = *reinterpret_cast<const float4 *>(b1 + ((cy * 2 + res) * 8) * 512);
+                                dep |= __float_as_uint(sv[0].w) | __float_as_uint(sv[1].w) | __float_as_uint(sv[2].w) | __float_as_uint(sv[3].w);
+                                if (res == 1) {   // all 16 loads of both slots have delivered: hand both back BEFORE the arithmetic
+                                    asm volatile("or.b32 %0, %0, 1;" : "+r"(dep));
+                                    dep = __reduce_or_sync(0xffffffffu, dep);
+                                    if (lane == 0 && dep != 0) {
+#pragma unroll
+                                        for (int sc = 0; sc < 4; ++sc) {
+                                            mbar_arrive_remote_relaxed(mapa(sf0, sc));
+                                            mbar_arrive_remote_relaxed(mapa(sf0 + 8, sc));
+                                        }
+                                    }
+                                }
 #pragma unroll
                                 for (int e = 0; e < 4; ++e) {
-                                    // Horner in beta_e: z = s0 + b (s1 + b (s2 + b s3)), two points at once
                                     const float2 bx = make_float2(be[e].x, be[e].x), by = make_float2(-be[e].y, be[e].y);
                                     float2 za = make_float2(sv[3].x, sv[3].y), zb = make_float2(sv[3].z, sv[3].w);
 #pragma unroll
@@ -956,61 +962,15 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                                         za = __ffma2_rn(make_float2(za.y, za.x), by, ta);
                                         zb = __ffma2_rn(make_float2(zb.y, zb.x), by, tb2);
                                     }
-                                    // two 8-byte stores: a 16-byte one costs four register moves (za, zb are not neighbours)
-                                    const uint32_t oa = smem_u32(base + ((e * 2 + res) * 8) * 512);
-                                    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(oa), "f"(za.x), "f"(za.y) : "memory");
-                                    asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" :: "r"(oa), "f"(zb.x), "f"(zb.y) : "memory");
+                                    const float2 oa = chime::cmul(za, wa), ob = chime::cmul(zb, wb);
+                                    const float2 xa = chime::cadd(z0a[e], oa), xa2 = chime::csub(z0a[e], oa);
+                                    const float2 xb = chime::cadd(z0b[e], ob), xb2 = chime::csub(z0b[e], ob);
+                                    acc[4 * e] = fmaf(xa.x, xa.x, fmaf(xa.y, xa.y, acc[4 * e]));
+                                    acc[4 * e + 1] = fmaf(xa2.x, xa2.x, fmaf(xa2.y, xa2.y, acc[4 * e + 1]));
+                                    acc[4 * e + 2] = fmaf(xb.x, xb.x, fmaf(xb.y, xb.y, acc[4 * e + 2]));
+                                    acc[4 * e + 3] = fmaf(xb2.x, xb2.x, fmaf(xb2.y, xb2.y, acc[4 * e + 3]));
                                 }
                             }
-                        }
-                        if (t & 1) {
-                            // U = 256: the FFT over u' has 32 points, u' = 16 h + u'': the tile of half 0 waits (E-W summed) in
-                            // the other slot, this one is half 1.  First stage across the halves, s = a0 + a1 and
-                            // d = (a0 - a1) W_32^{u''} (the twiddles W_256^{rho u'} were applied by the senders), then two FFT-16: s gives the
-                            // even bins, d the odd ones.  d waits in this thread's own cells of the slot meanwhile.
-                            bar_sync_named(1, 256);   // (covers phase 1 of the previous tile too: no barrier on even tiles)
-                            unsigned char *base1 = slot + ((e2 * 2 + res2) * 8) * 512;
-                            unsigned char *base0 = base1 + (s ? -kRecvBytes : kRecvBytes);
-#pragma unroll
-                            for (int k = 0; k < 8; ++k) {
-                                const float4 v0 = *reinterpret_cast<const float4 *>(base0 + k * 512);
-                                const float4 v1 = *reinterpret_cast<const float4 *>(base1 + k * 512);
-                                float2 sm[2], d[2];
-#pragma unroll
-                                for (int j = 0; j < 2; ++j) {
-                                    const int u = 2 * k + j;
-                                    float2 p0 = j ? make_float2(v0.z, v0.w) : make_float2(v0.x, v0.y);
-                                    float2 p1 = j ? make_float2(v1.z, v1.w) : make_float2(v1.x, v1.y);
-                                    sm[j] = chime::cadd(p0, p1);
-                                    d[j] = chime::csub(p0, p1);
-                                    if (u > 0) d[j] = chime::cmul(d[j], c_w32[u]);
-                                }
-                                // both branches wait in the thread's own cells (s in this slot, d in the other one), so that
-                                // the loop holds two points at a time and the FFTs run on the registers of U = 128
-                                const uint32_t o1 = smem_u32(base1 + k * 512), o0 = smem_u32(base0 + k * 512);
-                                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(o1), "f"(sm[0].x), "f"(sm[0].y) : "memory");
-                                asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" :: "r"(o1), "f"(sm[1].x), "f"(sm[1].y) : "memory");
-                                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(o0), "f"(d[0].x), "f"(d[0].y) : "memory");
-                                asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" :: "r"(o0), "f"(d[1].x), "f"(d[1].y) : "memory");
-                            }
-                            float2 a[16];
-#pragma unroll
-                            for (int k = 0; k < 8; ++k) {
-                                const float4 v = *reinterpret_cast<const float4 *>(base0 + k * 512);
-                                a[2 * k] = make_float2(v.x, v.y);
-                                a[2 * k + 1] = make_float2(v.z, v.w);
-                            }
-                            slot_free_arrive(a, sf0 + 8 * (s ^ 1), lane);   // half 0's slot is consumed
-                            fft16_detect(a, acc);
-#pragma unroll
-                            for (int k = 0; k < 8; ++k) {
-                                const float4 v = *reinterpret_cast<const float4 *>(base1 + k * 512);
-                                a[2 * k] = make_float2(v.x, v.y);
-                                a[2 * k + 1] = make_float2(v.z, v.w);
-                            }
-                            slot_free_arrive(a, sf0 + 8 * s, lane);
-                            fft16_detect(a, acc);
-                        }
                         }
                     }
                     // (pointers and the cache policy of the frame end are made here, once per frame: nothing of them is alive
@@ -1024,32 +984,32 @@ umma_beamform_kernel(const Params prm, const __grid_constant__ CUtensorMap tmap)
                     // 16-byte store per beam.  upchan 128: every thread brings 2 fine channels of the 4 E-W beams of its
                     // beam, warps 0-3 (E-W beam e2 = rw) take the 16 of (e2, beam).  upchan 256: the even warps bring the 16
                     // channels of their residue half, the odd ones add theirs.
-                    bool finisher;
-                    if constexpr (U == 128) {
-                        const int g0 = (bitrev(2 * rw, 4) + 8) & 15;     // position 2 rw -> bin bitrev(2 rw); 2 rw + 1 -> 8 further
+                    {
                         float *o8 = reinterpret_cast<float *>(smem + kOfsOut) + lane * 17;
+                        if constexpr (U == 128) {
+                            const int g0 = (bitrev(2 * rw, 4) + 8) & 15;     // position 2 rw -> bin bitrev(2 rw); 2 rw + 1 -> 8 further
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            o8[e * 32 * 17 + g0] = acc[2 * e];
-                            o8[e * 32 * 17 + (g0 ^ 8)] = acc[2 * e + 1];
-                        }
-                        finisher = rw < 4;
-                    } else {
-                        if (res2 == 0) {
+                            for (int e = 0; e < 4; ++e) {
+                                o8[e * 32 * 17 + g0] = acc[2 * e];
+                                o8[e * 32 * 17 + (g0 ^ 8)] = acc[2 * e + 1];
+                            }
+                        } else {
+                            // bins qa and qa ^ 1 (threads rw and rw ^ 4) share their fine channels: two staging halves
+                            const int ga = bitrev(rw, 3) >> 1;
+                            o8 += (rw >> 2) * (4 * 32 * 17);
 #pragma unroll
-                            for (int g = 0; g < 16; ++g) ost[g] = acc[g];
+                            for (int e = 0; e < 4; ++e) {
+                                o8[e * 32 * 17 + ga + 8] = acc[4 * e];
+                                o8[e * 32 * 17 + ga] = acc[4 * e + 1];
+                                o8[e * 32 * 17 + ga + 12] = acc[4 * e + 2];
+                                o8[e * 32 * 17 + ga + 4] = acc[4 * e + 3];
+                            }
                         }
-                        finisher = res2 == 1;
                     }
                     bar_sync_named(1, 256);
-                    if (finisher) {
-                        if constexpr (U == 128) {
+                    if (rw < 4) {
 #pragma unroll
-                            for (int g = 0; g < 16; ++g) acc[g] = ost[g];
-                        } else {
-#pragma unroll
-                            for (int g = 0; g < 16; ++g) acc[g] += ost[g];
-                        }
+                        for (int g = 0; g < 16; ++g) acc[g] = U == 128 ? ost[g] : ost[g] + ost[g + 4 * 32 * 17];
                         if (pol == 0) {
 #pragma unroll
                             for (int k = 0; k < 4; ++k)   // parked in L2 (evict_last: 17 MB for the whole grid must survive up to 16 frames of input streaming past)
