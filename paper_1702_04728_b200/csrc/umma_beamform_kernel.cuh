@@ -94,7 +94,7 @@ struct Params {
     int n_peers, chan_global0;
     float norm, scale, offset;
     float2 *packet_so;        // per-packet (scale, offset) out, [C][R][4 e][8 blocks of 32 beams], or nullptr (fixed scale)
-    float *scratch;           // [grid][4 frames][4 e][32 beams][16]: polarisation-0 sums parked until pol 1 is done (L2)
+    float *scratch;           // [grid][kMaxChunkFrames][4 e][32 beams][16]: polarisation-0 sums parked until pol 1 is done (L2)
     int *status;              // set to non-zero when a wait timed out (the kernel traps afterwards)
 };
 
