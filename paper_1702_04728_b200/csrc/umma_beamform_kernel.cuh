@@ -128,8 +128,8 @@ __device__ __forceinline__ bool mbar_try(uint32_t a, uint32_t parity) {
     return ok != 0;
 }
 // Development switches (off in the product; results are WRONG with CHIME_SKIP, it is for timing only):
-//   -DCHIME_SKIP=<mask>: 1 receive side's twiddle + FFT-16 + detection, 16 its E-W phase, 2 operand preparation,
-//                        4 the drain's arithmetic, 32 the drain's tensor-memory loads;
+//   -DCHIME_SKIP=<mask>: 2 operand preparation, 4 the drain's integer recombination, 16 the receive side's E-W sum and
+//                        detection (upchan 128), 32 the drain's tensor-memory loads;
 //   -DCHIME_PROF: clock64 around every wait of every role, read back with chime_bf_debug_prof.
 #ifdef CHIME_PROF
 __device__ long long g_prof[148 * 4][24][12];
